@@ -1,0 +1,95 @@
+"""CPU oracle for the Gatenby-Gawlinski finite-volume step -- TEST INFRASTRUCTURE, not product.
+
+Thin ctypes front for oracle/gg_oracle.cpp (plain fp64 C++, literal Table-1 / Table-2 stencils,
+eq. (3) of arXiv 2006.01748; see that file's header for citations and the pins that hold it).
+
+Only tests/, `__graft_entry__.smoke()` and bench.py's `cpu_baseline` / `--impl reference` legs may
+import this package.  It imports nothing from paper_2006_01748_b200 and is imported by nothing
+there.
+"""
+from __future__ import annotations
+
+import ctypes
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+_dp = ctypes.POINTER(ctypes.c_double)
+
+
+def load() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(_build.build())
+        lib.gg_oracle_D1.restype = ctypes.c_int
+        lib.gg_oracle_D1.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                     _dp, _dp, _dp]
+        lib.gg_oracle_D2.restype = ctypes.c_int
+        lib.gg_oracle_D2.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                     _dp, _dp, _dp, _dp, _dp]
+        lib.gg_oracle_step.restype = ctypes.c_int
+        lib.gg_oracle_step.argtypes = ([ctypes.c_int, ctypes.c_int] + [ctypes.c_double] * 6 +
+                                       [_dp] * 6 + [ctypes.c_longlong, ctypes.c_double,
+                                                    ctypes.c_int])
+        lib.gg_oracle_max_threads.restype = ctypes.c_int
+        lib.gg_oracle_max_threads.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def _c(x) -> np.ndarray:
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def _p(x: np.ndarray):
+    return x.ctypes.data_as(_dp)
+
+
+def max_threads() -> int:
+    return int(load().gg_oracle_max_threads())
+
+
+def D1(U, V, dx: float, dy: float) -> np.ndarray:
+    """D1(V;U), Table 1, mirrored ghosts.  U, V: [ny][nx]."""
+    U, V = _c(U), _c(V)
+    ny, nx = U.shape
+    out = np.empty_like(U)
+    rc = load().gg_oracle_D1(nx, ny, dx, dy, _p(U), _p(V), _p(out))
+    if rc != 0:
+        raise ValueError("gg_oracle_D1: bad argument")
+    return out
+
+
+def D2(a, b, c, W, dx: float, dy: float) -> np.ndarray:
+    """D2(W;A), Table 2, mirrored ghosts with b odd.  All [ny][nx]."""
+    a, b, c, W = _c(a), _c(b), _c(c), _c(W)
+    ny, nx = W.shape
+    out = np.empty_like(W)
+    rc = load().gg_oracle_D2(nx, ny, dx, dy, _p(a), _p(b), _p(c), _p(W), _p(out))
+    if rc != 0:
+        raise ValueError("gg_oracle_D2: bad argument")
+    return out
+
+
+def step(U, V, W, a, b, c, *, r: float, d: float, alpha: float, c_r: float, n: int, dt: float,
+         dx: float, dy: float | None = None, threads: int = 0):
+    """n explicit Euler steps of eq. (3).  Returns new (U, V, W); inputs untouched.
+
+    `c` is the tensor entry c_T(x,y) of eq. (2); `c_r` the reaction parameter eq. (1) calls c.
+    threads <= 0: all cores OpenMP sees (results are bit-identical for any thread count).
+    """
+    if dy is None:
+        dy = dx
+    U, V, W = _c(U).copy(), _c(V).copy(), _c(W).copy()
+    a, b, c = _c(a), _c(b), _c(c)
+    ny, nx = U.shape
+    for x in (V, W, a, b, c):
+        if x.shape != (ny, nx):
+            raise ValueError("shape mismatch")
+    rc = load().gg_oracle_step(nx, ny, dx, dy, r, d, alpha, c_r, _p(a), _p(b), _p(c), _p(U), _p(V),
+                               _p(W), int(n), float(dt), int(threads))
+    if rc != 0:
+        raise ValueError("gg_oracle_step: bad argument")
+    return U, V, W
