@@ -1,0 +1,155 @@
+/* gg.h -- C ABI of libgg.so: the explicit finite-volume step of the anisotropic, heterogeneous
+ * Gatenby-Gawlinski model (Mascia, Pera, Simeoni, arXiv 2006.01748) on one B200 (sm_100a).
+ *
+ * What the library computes (citations are lines of /root/reference/PAPER.md):
+ *   eq. (1)  PAPER.md:35     U_t = U(1-U) - d U W
+ *                            V_t = r V(1-V) + alpha div((1-U) grad V)
+ *                            W_t = c (V - W) + div(A grad W),   A = [[a,b],[b,c]]  (eq. (2), :40)
+ *   eq. (3)  PAPER.md:74     explicit Euler in time, every right-hand side at time level k;
+ *   Table 1  PAPER.md:81-85  five-point stencil D1(V;U), face diffusivity 1 - mean of adjacent U;
+ *   Table 2  PAPER.md:89-92  nine-point stencil D2(W;A), face means of a (x) and c (y), corner
+ *                            weights +-(b_{i+-1,j} + b_{i,j+-1})/(4 dx dy);
+ *   Neumann boundaries (no formula printed): DESIGN.md reading A2 -- mirror
+ *   extension across every boundary face with U,V,W,a,c even and b odd, i.e. zero total normal
+ *   flux through every boundary face and clamped neighbours in tangential differences.
+ * The kernels evaluate the stencils in flux form (each face flux once); the
+ * result equals the tables' up to floating-point evaluation order.  No clamping, no positivity
+ * fix, no NaN repair anywhere (eq. (3) has none).  No stability policing: dt is the caller's.
+ *
+ * The paper overloads `c`: gg_create's `c` is the reaction rate of eq. (1) (called c_r in
+ * DESIGN.md), gg_set_tensor's `c` is the tensor entry c(x,y) of eq. (2) (c_T).
+ *
+ * Layout.  Every field is row-major [ny][nx], x (index i) fastest: element (i,j) at j*nx + i;
+ * "right" is (i+1,j), "upper" is (i,j+1).  Batched states are [nbatch][ny][nx].
+ * Element type is the context's dtype (GG_F64: double, GG_F32: float) for state AND tensor.
+ * The nx x ny cells tile [0, nx*h] x [0, ny*h]; the domain boundary lies on cell faces.
+ *
+ * Memory.  The library never allocates device memory.  The caller allocates
+ * gg_workspace_bytes() bytes of device memory (256-byte aligned; a torch uint8 tensor will do)
+ * and hands it over with gg_bind; it must stay alive until gg_destroy.  All array arguments
+ * marked DEVICE are device pointers on the current CUDA device; HOST are host pointers.  The
+ * caller keeps ownership of every array it passes; the library copies in/out of its workspace.
+ *
+ * Streams.  Every call enqueues on the stream given to gg_bind (a cudaStream_t cast to void*,
+ * NULL = the legacy default stream) and returns without synchronising, except gg_destroy,
+ * gg_set_state_host/gg_get_state_host/gg_set_tensor_host (which synchronise that stream) and
+ * gg_last_step_ms.  Calls on one context must not be issued concurrently from several threads.
+ *
+ * Errors.  Every entry point returns GG_OK or an error code; nothing throws or aborts across the
+ * ABI.  gg_last_error gives a context-owned message for the last failing call (never freed by
+ * the caller; valid until the next call on that context).
+ */
+#ifndef GG_H_
+#define GG_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gg_ctx gg_ctx; /* opaque; one per simulation or per batch of simulations */
+
+enum { GG_F64 = 0, GG_F32 = 1 }; /* storage AND arithmetic type of state and tensor arrays */
+
+enum {
+    GG_OK = 0,
+    GG_ERR_ARG = 1,         /* null pointer, bad size, non-finite / non-positive h or dt, n < 0 */
+    GG_ERR_STATE = 2,       /* call order: step/get before bind + set_tensor + set_state */
+    GG_ERR_CUDA = 3,        /* CUDA runtime / driver failure; text in gg_last_error */
+    GG_ERR_UNSUPPORTED = 4  /* unknown dtype or option */
+};
+
+/* Kernel selection for gg_set_option(GG_OPT_KERNEL, .).  AUTO picks the fastest path that the
+ * shape allows; every path computes the same scheme. */
+enum {
+    GG_KERNEL_AUTO = 0,
+    GG_KERNEL_GENERIC = 1,  /* one thread per cell, global memory, clamp-indexed (any nx, ny)   */
+    GG_KERNEL_STREAM = 2,   /* TMA-staged shared-memory row ring, register-rolling y march;     */
+                            /* needs nx*sizeof(elem) % 16 == 0                                  */
+    GG_KERNEL_STREAM2 = 3,  /* as STREAM with two time steps fused per launch (temporal block)  */
+    GG_KERNEL_RESIDENT = 4  /* whole state resident on-chip across steps (small grids)          */
+};
+enum {
+    GG_OPT_KERNEL = 0,      /* one of GG_KERNEL_*                                               */
+    GG_OPT_GRAPH = 1,       /* 1 (default): step loop replayed from a cached CUDA graph; 0: plain launches */
+    GG_OPT_GRAPH_CHUNK = 2, /* steps per captured graph (default 64)                            */
+    GG_OPT_STREAM_VARIANT = 3,  /* tuning: which (rows/box, stages, warps/CTA) build of the STREAM
+                                   kernel runs; 0 .. gg_num_stream_variants()-1                  */
+    GG_OPT_ITEMS_PER_WARP = 4   /* tuning: target work items (row chunk x strip) per resident warp */
+};
+
+/* One simulation.  nx, ny >= 2 cells; h > 0 the mesh size (dx = dy = h);
+ * r, d, alpha, c the scalars of eq. (1); dtype GG_F64 or GG_F32.
+ * On success *out owns host-side resources only; free with gg_destroy. */
+int gg_create(gg_ctx** out, int nx, int ny, double h, double r, double d, double alpha, double c,
+              int dtype);
+
+/* nbatch >= 1 independent simulations on the same grid and the same tensor field, advanced
+ * together by every gg_step (the paper's "fast comparative simulations").
+ * r, d, alpha, c: HOST arrays [nbatch], copied. */
+int gg_create_batch(gg_ctx** out, int nbatch, int nx, int ny, double h, const double* r,
+                    const double* d, const double* alpha, const double* c, int dtype);
+
+/* Bytes of device memory the context needs: two copies of the state (ping-pong), one of the
+ * tensor, the per-simulation scalars, plus alignment padding.  0 if ctx is NULL. */
+size_t gg_workspace_bytes(const gg_ctx* ctx);
+
+/* Hand over caller-owned DEVICE memory (>= gg_workspace_bytes, 256-byte aligned) and the stream
+ * all later calls enqueue on.  Must be called once, before any set/step/get. */
+int gg_bind(gg_ctx* ctx, void* dev_workspace, size_t bytes, void* cuda_stream);
+
+/* Tensor field of eq. (2): a, b, c DEVICE arrays [ny][nx] of the context's dtype, cell-indexed
+ * like the unknowns; copied into the workspace.  Positive definiteness
+ * is assumed, not checked. */
+int gg_set_tensor(gg_ctx* ctx, const void* a, const void* b, const void* c);
+
+/* State at the current time level: U, V, W DEVICE arrays [nbatch][ny][nx]; copied. */
+int gg_set_state(gg_ctx* ctx, const void* U, const void* V, const void* W);
+
+/* n >= 0 explicit Euler steps of eq. (3) with constant step dt > 0.  All
+ * three fields advance together from time-k data only.  n == 0 is a no-op. */
+int gg_step(gg_ctx* ctx, long long n, double dt);
+
+/* Copy the current state (after every step issued so far) into DEVICE arrays [nbatch][ny][nx]. */
+int gg_get_state(gg_ctx* ctx, void* U, void* V, void* W);
+
+/* Host-buffer variants: the same calls with HOST arrays; the host<->device copies run on the
+ * bound stream and the call returns after they completed.  Pinned host memory copies fastest. */
+int gg_set_tensor_host(gg_ctx* ctx, const void* a, const void* b, const void* c);
+int gg_set_state_host(gg_ctx* ctx, const void* U, const void* V, const void* W);
+int gg_get_state_host(gg_ctx* ctx, void* U, void* V, void* W);
+
+/* Tuning / path selection; see GG_OPT_*.  Returns GG_ERR_UNSUPPORTED for an unknown option or a
+ * kernel the context's shape cannot run (the selection is never silently downgraded). */
+int gg_set_option(gg_ctx* ctx, int option, long long value);
+
+/* Introspection for benchmarks and tests.
+ * gg_kernel_used: GG_KERNEL_* the next gg_step will run (resolves AUTO), or -1.
+ * gg_launches:    number of step kernels this context has launched so far (graph replays count
+ *                 every kernel node).
+ * gg_last_step_ms: device time of the most recent gg_step call, measured with CUDA events
+ *                 recorded on the bound stream around its launches; synchronises on the end
+ *                 event.  *ms < 0 if no step has run. */
+int gg_kernel_used(const gg_ctx* ctx);
+long long gg_launches(const gg_ctx* ctx);
+int gg_last_step_ms(gg_ctx* ctx, float* ms);
+
+/* Synchronises the bound stream, releases graphs and host resources.  The workspace stays the
+ * caller's.  gg_destroy(NULL) is GG_OK. */
+int gg_destroy(gg_ctx* ctx);
+
+/* Message of the last failing call on ctx ("" if none); for ctx == NULL, the message of the
+ * last failing gg_create* on this thread. */
+const char* gg_last_error(const gg_ctx* ctx);
+
+/* Number of STREAM kernel builds selectable with GG_OPT_STREAM_VARIANT. */
+int gg_num_stream_variants(void);
+
+/* Library version string, e.g. "gg-b200 0.1 sm_100a". */
+const char* gg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GG_H_ */

@@ -1,0 +1,554 @@
+// gg_api.cu -- the C ABI of libgg.so (include/gg.h): context, argument validation, workspace
+// carving, tensor maps, kernel dispatch and the CUDA-graph step loop.  Product code; shares
+// nothing with oracle/.  Build: paper_2006_01748_b200/build.py (nvcc, sm_100a).
+#include "../../include/gg.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "gg_common.cuh"
+#include "gg_generic.cuh"
+#include "gg_stream.cuh"
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+thread_local std::string g_create_error;
+
+struct GraphKey {
+    long long len;
+    double dt;
+    int parity;
+    int kernel;
+    bool operator<(const GraphKey& o) const {
+        return std::tie(len, dt, parity, kernel) < std::tie(o.len, o.dt, o.parity, o.kernel);
+    }
+};
+
+}  // namespace
+
+struct gg_ctx {
+    int nx = 0, ny = 0, nbatch = 1, dtype = GG_F64;
+    double h = 0;
+    std::vector<gg::SimScalars> sims;
+    // workspace
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    bool bound = false, have_tensor = false, have_state = false;
+    void* state[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+    void* coef[3] = {nullptr, nullptr, nullptr};
+    gg::SimScalars* d_sims = nullptr;
+    int cur = 0;  // which ping-pong copy holds the current time level
+    // options
+    int opt_kernel = GG_KERNEL_AUTO;
+    int opt_graph = 1;
+    long long opt_chunk = 64;
+    int opt_variant = 0;
+    int opt_items_per_warp = 4;
+    // stream-kernel plan (tensor maps etc.)
+    gg::StreamPlan plan;
+    bool plan_ready = false;
+    // graphs
+    std::map<GraphKey, cudaGraphExec_t> graphs;
+    // stats
+    long long launches = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool timed = false;
+    int num_sms = 0;
+    mutable std::string err;
+
+    size_t esize() const { return dtype == GG_F64 ? 8 : 4; }
+    size_t plane() const { return (size_t)nx * ny; }
+};
+
+namespace {
+
+int fail(const gg_ctx* c, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf; else g_create_error = buf;
+    return code;
+}
+
+#define GG_CUDA(c, call)                                                                  \
+    do {                                                                                  \
+        cudaError_t e_ = (call);                                                          \
+        if (e_ != cudaSuccess)                                                            \
+            return fail((c), GG_ERR_CUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                              \
+    } while (0)
+
+struct Layout {
+    size_t state[2][3], coef[3], sims, total;
+};
+
+Layout layout_of(const gg_ctx* c) {
+    Layout L;
+    size_t off = 0;
+    const size_t sb = align_up((size_t)c->nbatch * c->plane() * c->esize());
+    const size_t cb = align_up(c->plane() * c->esize());
+    for (int p = 0; p < 2; ++p)
+        for (int f = 0; f < 3; ++f) { L.state[p][f] = off; off += sb; }
+    for (int f = 0; f < 3; ++f) { L.coef[f] = off; off += cb; }
+    L.sims = off;
+    off += align_up((size_t)c->nbatch * sizeof(gg::SimScalars));
+    L.total = off;
+    return L;
+}
+
+bool stream_shape_ok(const gg_ctx* c) { return ((size_t)c->nx * c->esize()) % 16 == 0; }
+
+int resolve_kernel(const gg_ctx* c) {
+    if (c->opt_kernel != GG_KERNEL_AUTO) return c->opt_kernel;
+    return stream_shape_ok(c) ? GG_KERNEL_STREAM : GG_KERNEL_GENERIC;
+}
+
+void drop_graphs(gg_ctx* c) {
+    for (auto& kv : c->graphs) cudaGraphExecDestroy(kv.second);
+    c->graphs.clear();
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// Stream-kernel plan: tensor maps + launch geometry
+// ------------------------------------------------------------------------------------------
+namespace {
+
+// Stream kernel instantiations (rows per TMA box, ring stages per warp, warps per CTA); the
+// default is the one tuned on B200, the others stay selectable through
+// GG_OPT_STREAM_VARIANT for re-tuning.
+struct Variant { int rb, nst, nw; };
+constexpr Variant kVariants[] = {{2, 3, 10}, {2, 2, 16}, {4, 2, 8}, {2, 4, 8}, {1, 3, 16}, {1, 4, 12}};
+constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
+constexpr int kDefaultVariant = 0;
+
+// Calls F.template operator()<T, RB, NST, NW>() for variant v.
+template <typename T, typename F>
+int with_variant(int v, F&& f) {
+    switch (v) {
+        case 0: return f.template operator()<T, 2, 3, 10>();
+        case 1: return f.template operator()<T, 2, 2, 16>();
+        case 2: return f.template operator()<T, 4, 2, 8>();
+        case 3: return f.template operator()<T, 2, 4, 8>();
+        case 4: return f.template operator()<T, 1, 3, 16>();
+        case 5: return f.template operator()<T, 1, 4, 12>();
+    }
+    return -1;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) !=
+                cudaSuccess || qres != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return (EncodeTiledFn)p;
+    }();
+    return fn;
+}
+
+int make_map(gg_ctx* c, CUtensorMap* m, void* base, int depth, int box_rows) {
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return fail(c, GG_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+    const size_t es = c->esize();
+    cuuint64_t dims[3] = {(cuuint64_t)c->nx, (cuuint64_t)c->ny, (cuuint64_t)depth};
+    cuuint64_t strides[2] = {(cuuint64_t)c->nx * es, (cuuint64_t)c->plane() * es};
+    cuuint32_t box[3] = {(cuuint32_t)(gg::kRowBytes / es), (cuuint32_t)box_rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(m, c->dtype == GG_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64
+                                           : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                     3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(c, GG_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return GG_OK;
+}
+
+struct KernelPtr {
+    const void** out;
+    template <typename T, int RB, int NST, int NW>
+    int operator()() const { *out = (const void*)gg::gg_step_stream<T, RB, NST, NW>; return 0; }
+};
+struct KernelLaunch {
+    const gg::StreamPlan* P;
+    const gg::StreamArgs* a;
+    cudaStream_t stream;
+    template <typename T, int RB, int NST, int NW>
+    int operator()() const {
+        gg::gg_step_stream<T, RB, NST, NW><<<P->grid, P->block, P->smem, stream>>>(*a);
+        return 0;
+    }
+};
+
+int build_plan(gg_ctx* c) {
+    if (c->plan_ready) return GG_OK;
+    if (!stream_shape_ok(c))
+        return fail(c, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0");
+    gg::StreamPlan& P = c->plan;
+    const Variant var = kVariants[c->opt_variant];
+    const int kRB = var.rb, kNST = var.nst, kNW = var.nw;
+    for (int p = 0; p < 2; ++p)
+        for (int f = 0; f < 3; ++f) {
+            int rc = make_map(c, &P.state[p][f], c->state[p][f], c->nbatch, kRB);
+            if (rc) return rc;
+        }
+    for (int f = 0; f < 3; ++f) {
+        int rc = make_map(c, &P.coef[f], c->coef[f], 1, kRB);
+        if (rc) return rc;
+    }
+    const int strip_cells = gg::kStripBytes / (int)c->esize();
+    P.nstrips = (c->nx + strip_cells - 1) / strip_cells;
+    P.rb = kRB; P.nst = kNST; P.nw = kNW;
+    P.block = kNW * 32;
+    P.smem = (size_t)((kNW * kNST * 8 + 127) / 128 * 128) +
+             (size_t)kNW * kNST * 6 * ((kRB * gg::kRowBytes + 127) / 128 * 128);
+    const void* fn = nullptr;
+    if (c->dtype == GG_F64) with_variant<double>(c->opt_variant, KernelPtr{&fn});
+    else with_variant<float>(c->opt_variant, KernelPtr{&fn});
+    GG_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem));
+    // Row chunks: enough items that every warp of a full grid gets several, none shorter than
+    // 16 rows (the two halo rows per chunk are re-read, from L2 when neighbours run together).
+    const long long warps = (long long)c->num_sms * kNW;
+    long long want = (long long)c->opt_items_per_warp * warps;  // target items
+    long long per = (long long)P.nstrips * c->nbatch;
+    long long nchunks = (want + per - 1) / per;
+    long long max_chunks = (c->ny + 15) / 16;
+    if (nchunks > max_chunks) nchunks = max_chunks;
+    if (nchunks < 1) nchunks = 1;
+    P.chunk_rows = (int)((c->ny + nchunks - 1) / nchunks);
+    P.nchunks = (c->ny + P.chunk_rows - 1) / P.chunk_rows;
+    P.nitems = (long long)P.nstrips * P.nchunks * c->nbatch;
+    long long ctas = (P.nitems + kNW - 1) / kNW;
+    P.grid = (int)(ctas < c->num_sms ? ctas : c->num_sms);
+    c->plan_ready = true;
+    return GG_OK;
+}
+
+template <typename T>
+int launch_generic(gg_ctx* c, int src, double dt) {
+    gg::GenericArgs<T> a;
+    a.U = (const T*)c->state[src][0]; a.V = (const T*)c->state[src][1]; a.W = (const T*)c->state[src][2];
+    a.U1 = (T*)c->state[src ^ 1][0]; a.V1 = (T*)c->state[src ^ 1][1]; a.W1 = (T*)c->state[src ^ 1][2];
+    a.a = (const T*)c->coef[0]; a.b = (const T*)c->coef[1]; a.c = (const T*)c->coef[2];
+    a.sims = c->d_sims;
+    a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
+    a.dt = dt; a.inv_h2 = 1.0 / (c->h * c->h);
+    dim3 block(64, 4, 1);
+    dim3 grid((c->nx + 63) / 64, (c->ny + 3) / 4, c->nbatch);
+    gg::gg_step_generic<T><<<grid, block, 0, c->stream>>>(a);
+    GG_CUDA(c, cudaGetLastError());
+    return GG_OK;
+}
+
+int launch_stream(gg_ctx* c, int src, double dt) {
+    const gg::StreamPlan& P = c->plan;
+    gg::StreamArgs a;
+    a.mU = P.state[src][0]; a.mV = P.state[src][1]; a.mW = P.state[src][2];
+    a.ma = P.coef[0]; a.mb = P.coef[1]; a.mc = P.coef[2];
+    a.U1 = c->state[src ^ 1][0]; a.V1 = c->state[src ^ 1][1]; a.W1 = c->state[src ^ 1][2];
+    a.sims = c->d_sims;
+    a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
+    a.nstrips = P.nstrips; a.nchunks = P.nchunks; a.chunk_rows = P.chunk_rows;
+    a.nitems = P.nitems;
+    a.dt = dt; a.inv_h2 = 1.0 / (c->h * c->h);
+    if (c->dtype == GG_F64) with_variant<double>(c->opt_variant, KernelLaunch{&P, &a, c->stream});
+    else with_variant<float>(c->opt_variant, KernelLaunch{&P, &a, c->stream});
+    GG_CUDA(c, cudaGetLastError());
+    return GG_OK;
+}
+
+// one step from ping-pong copy `src` into `src^1`
+int launch_step(gg_ctx* c, int kernel, int src, double dt) {
+    switch (kernel) {
+        case GG_KERNEL_GENERIC:
+            return c->dtype == GG_F64 ? launch_generic<double>(c, src, dt)
+                                      : launch_generic<float>(c, src, dt);
+        case GG_KERNEL_STREAM:
+            return launch_stream(c, src, dt);
+        default:
+            return fail(c, GG_ERR_UNSUPPORTED, "kernel %d not available", kernel);
+    }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// extern "C" entry points (contracts in include/gg.h)
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+int gg_create_batch(gg_ctx** out, int nbatch, int nx, int ny, double h, const double* r,
+                    const double* d, const double* alpha, const double* c, int dtype) {
+    if (!out) return fail(nullptr, GG_ERR_ARG, "gg_create: out is NULL");
+    *out = nullptr;
+    if (nbatch < 1) return fail(nullptr, GG_ERR_ARG, "gg_create: nbatch %d < 1", nbatch);
+    if (nx < 2 || ny < 2) return fail(nullptr, GG_ERR_ARG, "gg_create: nx, ny must be >= 2 (got %d x %d)", nx, ny);
+    if (!(h > 0.0) || !std::isfinite(h)) return fail(nullptr, GG_ERR_ARG, "gg_create: h must be finite and > 0");
+    if (!r || !d || !alpha || !c) return fail(nullptr, GG_ERR_ARG, "gg_create: NULL parameter array");
+    if (dtype != GG_F64 && dtype != GG_F32) return fail(nullptr, GG_ERR_UNSUPPORTED, "gg_create: unknown dtype %d", dtype);
+    if ((double)nx * ny * nbatch > 2.0e10) return fail(nullptr, GG_ERR_ARG, "gg_create: grid too large");
+    for (int s = 0; s < nbatch; ++s)
+        if (!std::isfinite(r[s]) || !std::isfinite(d[s]) || !std::isfinite(alpha[s]) || !std::isfinite(c[s]))
+            return fail(nullptr, GG_ERR_ARG, "gg_create: non-finite parameter for simulation %d", s);
+    gg_ctx* ctx = new (std::nothrow) gg_ctx;
+    if (!ctx) return fail(nullptr, GG_ERR_ARG, "gg_create: out of host memory");
+    ctx->nx = nx; ctx->ny = ny; ctx->nbatch = nbatch; ctx->h = h; ctx->dtype = dtype;
+    ctx->sims.resize(nbatch);
+    for (int s = 0; s < nbatch; ++s) ctx->sims[s] = gg::SimScalars{r[s], d[s], alpha[s], c[s]};
+    ctx->opt_variant = kDefaultVariant;
+    *out = ctx;
+    return GG_OK;
+}
+
+int gg_create(gg_ctx** out, int nx, int ny, double h, double r, double d, double alpha, double c,
+              int dtype) {
+    return gg_create_batch(out, 1, nx, ny, h, &r, &d, &alpha, &c, dtype);
+}
+
+size_t gg_workspace_bytes(const gg_ctx* ctx) { return ctx ? layout_of(ctx).total : 0; }
+
+int gg_bind(gg_ctx* ctx, void* ws, size_t bytes, void* stream) {
+    if (!ctx) return GG_ERR_ARG;
+    if (ctx->bound) return fail(ctx, GG_ERR_STATE, "gg_bind: already bound");
+    if (!ws) return fail(ctx, GG_ERR_ARG, "gg_bind: workspace is NULL");
+    const Layout L = layout_of(ctx);
+    if (bytes < L.total) return fail(ctx, GG_ERR_ARG, "gg_bind: workspace %zu B < required %zu B", bytes, L.total);
+    if ((uintptr_t)ws % kAlign) return fail(ctx, GG_ERR_ARG, "gg_bind: workspace not 256-byte aligned");
+    cudaPointerAttributes at;
+    GG_CUDA(ctx, cudaPointerGetAttributes(&at, ws));
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+        return fail(ctx, GG_ERR_ARG, "gg_bind: workspace is not device memory");
+    int dev = 0;
+    GG_CUDA(ctx, cudaGetDevice(&dev));
+    GG_CUDA(ctx, cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    ctx->ws = (char*)ws; ctx->ws_bytes = bytes; ctx->stream = (cudaStream_t)stream;
+    for (int p = 0; p < 2; ++p)
+        for (int f = 0; f < 3; ++f) ctx->state[p][f] = ctx->ws + L.state[p][f];
+    for (int f = 0; f < 3; ++f) ctx->coef[f] = ctx->ws + L.coef[f];
+    ctx->d_sims = (gg::SimScalars*)(ctx->ws + L.sims);
+    GG_CUDA(ctx, cudaMemcpyAsync(ctx->d_sims, ctx->sims.data(), ctx->sims.size() * sizeof(gg::SimScalars),
+                                 cudaMemcpyHostToDevice, ctx->stream));
+    GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // sims is pageable host memory
+    GG_CUDA(ctx, cudaEventCreate(&ctx->ev0));
+    GG_CUDA(ctx, cudaEventCreate(&ctx->ev1));
+    ctx->bound = true;
+    return GG_OK;
+}
+
+static int copy3(gg_ctx* ctx, void* const dst[3], const void* const src[3], size_t bytes,
+                 cudaMemcpyKind kind, bool sync) {
+    for (int f = 0; f < 3; ++f)
+        GG_CUDA(ctx, cudaMemcpyAsync(dst[f], src[f], bytes, kind, ctx->stream));
+    if (sync) GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return GG_OK;
+}
+
+static int set_tensor_impl(gg_ctx* ctx, const void* a, const void* b, const void* c, bool host) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound) return fail(ctx, GG_ERR_STATE, "gg_set_tensor: call gg_bind first");
+    if (!a || !b || !c) return fail(ctx, GG_ERR_ARG, "gg_set_tensor: NULL array");
+    const void* src[3] = {a, b, c};
+    int rc = copy3(ctx, ctx->coef, src, ctx->plane() * ctx->esize(),
+                   host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, host);
+    if (rc) return rc;
+    ctx->have_tensor = true;
+    return GG_OK;
+}
+static int set_state_impl(gg_ctx* ctx, const void* U, const void* V, const void* W, bool host) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound) return fail(ctx, GG_ERR_STATE, "gg_set_state: call gg_bind first");
+    if (!U || !V || !W) return fail(ctx, GG_ERR_ARG, "gg_set_state: NULL array");
+    const void* src[3] = {U, V, W};
+    int rc = copy3(ctx, ctx->state[ctx->cur], src, (size_t)ctx->nbatch * ctx->plane() * ctx->esize(),
+                   host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, host);
+    if (rc) return rc;
+    ctx->have_state = true;
+    return GG_OK;
+}
+static int get_state_impl(gg_ctx* ctx, void* U, void* V, void* W, bool host) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound || !ctx->have_state) return fail(ctx, GG_ERR_STATE, "gg_get_state: no state set");
+    if (!U || !V || !W) return fail(ctx, GG_ERR_ARG, "gg_get_state: NULL array");
+    void* dst[3] = {U, V, W};
+    return copy3(ctx, dst, ctx->state[ctx->cur], (size_t)ctx->nbatch * ctx->plane() * ctx->esize(),
+                 host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, host);
+}
+
+int gg_set_tensor(gg_ctx* c, const void* a, const void* b, const void* cc) { return set_tensor_impl(c, a, b, cc, false); }
+int gg_set_tensor_host(gg_ctx* c, const void* a, const void* b, const void* cc) { return set_tensor_impl(c, a, b, cc, true); }
+int gg_set_state(gg_ctx* c, const void* U, const void* V, const void* W) { return set_state_impl(c, U, V, W, false); }
+int gg_set_state_host(gg_ctx* c, const void* U, const void* V, const void* W) { return set_state_impl(c, U, V, W, true); }
+int gg_get_state(gg_ctx* c, void* U, void* V, void* W) { return get_state_impl(c, U, V, W, false); }
+int gg_get_state_host(gg_ctx* c, void* U, void* V, void* W) { return get_state_impl(c, U, V, W, true); }
+
+}  // extern "C"
+
+namespace {
+
+// Capture `len` consecutive steps starting from ping-pong copy `src` into an executable graph.
+int capture_graph(gg_ctx* c, int kernel, long long len, double dt, int src, cudaGraphExec_t* out) {
+    cudaStream_t cap = nullptr;
+    GG_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = c->stream;
+    c->stream = cap;  // launch_step enqueues on c->stream
+    cudaGraph_t graph = nullptr;
+    int rc = GG_OK;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) {
+        rc = fail(c, GG_ERR_CUDA, "cudaStreamBeginCapture: %s", cudaGetErrorString(e));
+    } else {
+        int s = src;
+        for (long long k = 0; k < len && rc == GG_OK; ++k, s ^= 1) rc = launch_step(c, kernel, s, dt);
+        e = cudaStreamEndCapture(cap, &graph);
+        if (rc == GG_OK && e != cudaSuccess)
+            rc = fail(c, GG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    }
+    c->stream = user;
+    if (rc == GG_OK) {
+        e = cudaGraphInstantiate(out, graph, 0);
+        if (e != cudaSuccess) rc = fail(c, GG_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+    }
+    if (graph) cudaGraphDestroy(graph);
+    cudaStreamDestroy(cap);
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gg_step(gg_ctx* ctx, long long n, double dt) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound || !ctx->have_tensor || !ctx->have_state)
+        return fail(ctx, GG_ERR_STATE, "gg_step: needs gg_bind, gg_set_tensor and gg_set_state first");
+    if (n < 0) return fail(ctx, GG_ERR_ARG, "gg_step: n = %lld < 0", n);
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
+    if (n == 0) return GG_OK;
+    const int kernel = resolve_kernel(ctx);
+    if (kernel == GG_KERNEL_STREAM) {
+        int rc = build_plan(ctx);
+        if (rc) return rc;
+    }
+    GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+    long long left = n;
+    if (ctx->opt_graph && n >= 2) {
+        const long long chunk = ctx->opt_chunk;
+        while (left > 0) {
+            const long long len = left < chunk ? left : chunk;
+            const GraphKey key{len, dt, ctx->cur, kernel};
+            auto it = ctx->graphs.find(key);
+            if (it == ctx->graphs.end()) {
+                if (ctx->graphs.size() >= 32) drop_graphs(ctx);
+                cudaGraphExec_t ex = nullptr;
+                int rc = capture_graph(ctx, kernel, len, dt, ctx->cur, &ex);
+                if (rc) return rc;
+                it = ctx->graphs.emplace(key, ex).first;
+            }
+            GG_CUDA(ctx, cudaGraphLaunch(it->second, ctx->stream));
+            ctx->cur ^= (int)(len & 1);
+            ctx->launches += len;
+            left -= len;
+        }
+    } else {
+        for (; left > 0; --left) {
+            int rc = launch_step(ctx, kernel, ctx->cur, dt);
+            if (rc) return rc;
+            ctx->cur ^= 1;
+            ctx->launches += 1;
+        }
+    }
+    GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+    ctx->timed = true;
+    return GG_OK;
+}
+
+int gg_set_option(gg_ctx* ctx, int option, long long value) {
+    if (!ctx) return GG_ERR_ARG;
+    switch (option) {
+        case GG_OPT_KERNEL:
+            if (value == GG_KERNEL_AUTO || value == GG_KERNEL_GENERIC) break;
+            if (value == GG_KERNEL_STREAM) {
+                if (!stream_shape_ok(ctx))
+                    return fail(ctx, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0 (nx = %d)", ctx->nx);
+                break;
+            }
+            return fail(ctx, GG_ERR_UNSUPPORTED, "gg_set_option: kernel %lld not available", value);
+        case GG_OPT_GRAPH:
+            if (value != 0 && value != 1) return fail(ctx, GG_ERR_ARG, "GG_OPT_GRAPH: 0 or 1");
+            break;
+        case GG_OPT_GRAPH_CHUNK:
+            if (value < 1 || value > 4096) return fail(ctx, GG_ERR_ARG, "GG_OPT_GRAPH_CHUNK: 1..4096");
+            break;
+        case GG_OPT_STREAM_VARIANT:
+            if (value < 0 || value >= kNumVariants) return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_VARIANT: 0..%d", kNumVariants - 1);
+            break;
+        case GG_OPT_ITEMS_PER_WARP:
+            if (value < 1 || value > 1024) return fail(ctx, GG_ERR_ARG, "GG_OPT_ITEMS_PER_WARP: 1..1024");
+            break;
+        default:
+            return fail(ctx, GG_ERR_UNSUPPORTED, "gg_set_option: unknown option %d", option);
+    }
+    drop_graphs(ctx);
+    switch (option) {
+        case GG_OPT_KERNEL: ctx->opt_kernel = (int)value; break;
+        case GG_OPT_GRAPH: ctx->opt_graph = (int)value; break;
+        case GG_OPT_GRAPH_CHUNK: ctx->opt_chunk = value; break;
+        case GG_OPT_STREAM_VARIANT: ctx->opt_variant = (int)value; ctx->plan_ready = false; break;
+        case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = false; break;
+    }
+    return GG_OK;
+}
+
+int gg_kernel_used(const gg_ctx* ctx) { return ctx ? resolve_kernel(ctx) : -1; }
+long long gg_launches(const gg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int gg_last_step_ms(gg_ctx* ctx, float* ms) {
+    if (!ctx || !ms) return GG_ERR_ARG;
+    *ms = -1.0f;
+    if (!ctx->timed) return GG_OK;
+    GG_CUDA(ctx, cudaEventSynchronize(ctx->ev1));
+    GG_CUDA(ctx, cudaEventElapsedTime(ms, ctx->ev0, ctx->ev1));
+    return GG_OK;
+}
+
+int gg_destroy(gg_ctx* ctx) {
+    if (!ctx) return GG_OK;
+    int rc = GG_OK;
+    if (ctx->bound) {
+        if (cudaStreamSynchronize(ctx->stream) != cudaSuccess) rc = GG_ERR_CUDA;
+        drop_graphs(ctx);
+        if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+        if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    }
+    delete ctx;
+    return rc;
+}
+
+const char* gg_last_error(const gg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+int gg_num_stream_variants(void) { return kNumVariants; }
+const char* gg_version(void) { return "gg-b200 0.1 sm_100a"; }
+
+}  // extern "C"
