@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused finite-volume step on B200 (contract in DESIGN.md section 8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--extras]
+
+A "step" is one explicit time step of the whole hot path (U, V and W updated together, eq. (3) of
+arXiv 2006.01748) over BASELINE.json's headline workload: config 3, 8192 x 8192 cells, fp64,
+layered discontinuous tensor, three tumour disks (synthetic, seeded: workloads.make(3)).
+
+Prints ONE JSON line on stdout:
+  value         cell-updates/s in GLUPS, whole job, inputs resident in HBM, K steps timed on the
+                device (CUDA events recorded by libgg on its stream around the K launches)
+  e2e           the same metric through the C ABI with HOST (pinned) buffers: upload tensor and
+                state, K steps, download state, all inside the timed region
+  roofline      compulsory bytes (72 B per cell-update in fp64) / measured launch time against the
+                measured HBM copy peak (MEASURED_PEAKS.json)
+  cpu_baseline  the CPU oracle, as it stands, on a bounded sample of the same workload
+N > 1 (torchrun): the path does not shard without a halo exchange that north_star excludes, so
+every rank runs an independent replica of the same workload ("replicas only", weak scaling);
+value = all ranks' cell-updates / max-over-ranks device time.
+`--impl reference` times the oracle (the reference arm of this tier) on rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/s, explicit finite-volume step, fp64 8192^2 (BASELINE config 3)"
+UNIT = "GLUPS"
+BYTES_PER_CELL = {"f64": 72.0, "f32": 36.0}   # 3 fields read + 3 written + 3 coefficients read
+FALLBACK_HBM_GBS = 6650.0                      # /opt/skills/guides/B200_PROFILING.md
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(dtype):
+    """Per-launch DRAM bytes of the step kernel from the committed ncu capture, or None."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))[dtype])
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clock / throttle-reason samples while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline / --impl reference): the oracle as it stands, bounded sample
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(wl, rows=1024, steps=4):
+    """Time `steps` oracle steps on the first `rows` rows of the workload (full width, so the
+    memory access pattern per row is the workload's).  Returns (GLUPS, description, threads)."""
+    import oracle
+    rows = min(rows, wl.ny)
+    sl = slice(0, rows)
+    U, V, W = wl.U[0, sl], wl.V[0, sl], wl.W[0, sl]
+    a, b, c = wl.a[sl], wl.b[sl], wl.c[sl]
+    kw = dict(r=wl.r[0], d=wl.d[0], alpha=wl.alpha[0], c_r=wl.c_r[0], dt=wl.dt, dx=wl.h)
+    oracle.step(U, V, W, a, b, c, n=1, **kw)  # warm-up (page faults, library load)
+    t0 = time.perf_counter()
+    oracle.step(U, V, W, a, b, c, n=steps, **kw)
+    t = time.perf_counter() - t0
+    glups = rows * wl.nx * steps / t / 1e9
+    desc = (f"oracle/gg_oracle.cpp (fp64, OpenMP over rows), {steps} steps on rows 0..{rows - 1} "
+            f"x all {wl.nx} columns of {wl.name}, {t:.2f} s")
+    return glups, desc, oracle.max_threads(), t
+
+
+def run_reference(args, wl):
+    """Reference arm of this tier = the CPU oracle; K 'steps' are K oracle steps on the sample."""
+    import oracle
+    rows = 256                  # bounded: K steps at ~15 M cell-updates/s must end in minutes
+    sl = slice(0, rows)
+    U, V, W = wl.U[0, sl], wl.V[0, sl], wl.W[0, sl]
+    a, b, c = wl.a[sl], wl.b[sl], wl.c[sl]
+    kw = dict(r=wl.r[0], d=wl.d[0], alpha=wl.alpha[0], c_r=wl.c_r[0], dt=wl.dt, dx=wl.h)
+    K = min(args.steps, 400)
+    Wm = min(args.warmup, 3)
+    oracle.step(U, V, W, a, b, c, n=max(Wm, 1), **kw)
+    t0 = time.perf_counter()
+    oracle.step(U, V, W, a, b, c, n=K, **kw)
+    t = time.perf_counter() - t0
+    glups = rows * wl.nx * K / t / 1e9
+    sample = (f"{K} oracle steps on rows 0..{rows - 1} x all {wl.nx} columns of {wl.name} "
+              f"(bounded sample of the 8192^2 workload)")
+    return {
+        "impl": "reference", "metric": METRIC, "value": glups, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": K, "warmup": Wm, "ms_per_step": t / K * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[3]: 8192x8192 fp64 layered tensor, 3 disks",
+                   "sample": sample},
+        "cpu_baseline": {"value": glups, "unit": UNIT, "cores": oracle.max_threads(),
+                         "kind": "oracle", "sample": sample},
+        "e2e": {"value": glups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+# ---------------------------------------------------------------------------------------------
+# GPU leg
+# ---------------------------------------------------------------------------------------------
+def run_ours(args, wl, rank, world, device):
+    import torch
+    from paper_2006_01748_b200 import binding
+
+    dtype = args.dtype
+    npd = np.float64 if dtype == "f64" else np.float32
+    K, Wm = args.steps, max(args.warmup, 3)
+    cells = wl.nx * wl.ny * wl.batch
+    dist = world > 1
+    if dist:
+        import torch.distributed as td
+
+    def barrier():
+        if dist:
+            td.barrier()
+        torch.cuda.synchronize(device)
+
+    def max_over_ranks(x):
+        if not dist:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        td.all_reduce(t, op=td.ReduceOp.MAX)
+        return float(t.item())
+
+    sim = binding.Simulation(wl.nx, wl.ny, wl.h, wl.r, wl.d, wl.alpha, wl.c_r, dtype=dtype,
+                             batch=wl.batch, device=str(device))
+    if args.kernel:
+        sim.set_option(binding.GG_OPT_KERNEL, {"generic": 1, "stream": 2}[args.kernel])
+    # pinned host copies of the inputs (what a host-side caller holds)
+    host = {k: torch.from_numpy(np.ascontiguousarray(getattr(wl, k), dtype=npd)).pin_memory()
+            for k in ("a", "b", "c", "U", "V", "W")}
+    out = {k: torch.empty_like(host[k]).pin_memory() for k in ("U", "V", "W")}
+    ptr = lambda t: t.data_ptr()
+    binding.gg_set_tensor_host(sim.ctx, ptr(host["a"]), ptr(host["b"]), ptr(host["c"]))
+    binding.gg_set_state_host(sim.ctx, ptr(host["U"]), ptr(host["V"]), ptr(host["W"]))
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps -----------------------
+    sim.step(Wm, wl.dt)
+    sim.step(K, wl.dt)          # builds and caches the K-step graphs (untimed)
+    binding.gg_set_state_host(sim.ctx, ptr(host["U"]), ptr(host["V"]), ptr(host["W"]))
+    l0 = sim.launches
+    barrier()
+    with ClockSampler(device.index or 0) as clk:
+        reps = []
+        for _ in range(args.reps):
+            barrier()
+            sim.step(K, wl.dt)
+            reps.append(sim.last_step_ms())   # CUDA events on libgg's stream around the K launches
+            barrier()
+    launches = (sim.launches - l0) // args.reps
+    ms = max_over_ranks(float(np.median(reps)))
+    value = cells * world * K / (ms * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with host buffers --------------------------------------
+    barrier()
+    t0 = time.perf_counter()
+    binding.gg_set_tensor_host(sim.ctx, ptr(host["a"]), ptr(host["b"]), ptr(host["c"]))
+    binding.gg_set_state_host(sim.ctx, ptr(host["U"]), ptr(host["V"]), ptr(host["W"]))
+    sim.step(K, wl.dt)
+    binding.gg_get_state_host(sim.ctx, ptr(out["U"]), ptr(out["V"]), ptr(out["W"]))
+    torch.cuda.synchronize(device)
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    es = 8 if dtype == "f64" else 4
+    h2d = (3 * wl.nx * wl.ny + 3 * cells) * es
+    d2h = 3 * cells * es
+    e2e = {"value": cells * world * K / e2e_s / 1e9, "unit": UNIT,
+           "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+           "what": f"gg_set_tensor_host + gg_set_state_host + gg_step({K}) + gg_get_state_host, "
+                   f"pinned host buffers, {h2d / 1e9:.2f} GB up and {d2h / 1e9:.2f} GB down per job",
+           "seconds": e2e_s}
+    final = tuple(out[k].numpy() for k in ("U", "V", "W"))
+    kernel = sim.kernel
+    sim.close()
+    return dict(value=value, ms=ms / K, reps_ms=reps, launches=launches, e2e=e2e,
+                clocks=clk.summary(), kernel=kernel, final=final)
+
+
+def sampled_parity(wl, final, K, size=48):
+    """Oracle check of the e2e end state on two windows the oracle can afford: the domain corner
+    (true Neumann faces on two sides) and a window on the rim of the first tumour disk.  A window
+    is cut with a margin of K cells on its interior sides (the stencil moves information one cell
+    per step), the oracle runs K steps on the cut, and only the uncontaminated core is compared."""
+    import oracle
+    x, y = np.meshgrid(np.arange(wl.nx), np.arange(wl.ny), indexing="xy")
+    inside = wl.V[0] > 0.5
+    jj, ii = np.nonzero(inside)
+    k = np.argmin(ii)  # leftmost cell of a disk: a front
+    spots = {"corner": (0, 0), "front": (max(int(ii[k]) - size // 2, 0), max(int(jj[k]) - size // 2, 0))}
+    del x, y
+    worst = 0.0
+    for name, (i0, j0) in spots.items():
+        ia, ja = max(i0 - K, 0), max(j0 - K, 0)
+        ib, jb = min(i0 + size + K, wl.nx), min(j0 + size + K, wl.ny)
+        cut = (slice(ja, jb), slice(ia, ib))
+        ref = oracle.step(wl.U[0][cut], wl.V[0][cut], wl.W[0][cut], wl.a[cut], wl.b[cut], wl.c[cut],
+                          r=wl.r[0], d=wl.d[0], alpha=wl.alpha[0], c_r=wl.c_r[0], n=K, dt=wl.dt,
+                          dx=wl.h)
+        core = (slice(j0 - ja, j0 - ja + size), slice(i0 - ia, i0 - ia + size))
+        full = (slice(j0, j0 + size), slice(i0, i0 + size))
+        for f in range(3):
+            worst = max(worst, float(np.max(np.abs(final[f][0][full].astype(np.float64) - ref[f][core]))))
+    return worst
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--kernel", default=None, choices=[None, "generic", "stream"])
+    ap.add_argument("--reps", type=int, default=3)
+    ap.add_argument("--n", type=int, default=8192, help="grid edge (8192 = the headline config)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2006_01748_b200 import workloads
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        wl = workloads.make(3, nx=args.n, ny=args.n)
+        print(json.dumps(run_reference(args, wl)), flush=True)
+        return 0
+
+    import torch
+    if not torch.cuda.is_available():
+        log("bench.py: no CUDA device; the product has no CPU fallback")
+        return 2
+    device = torch.device("cuda", local)
+    torch.cuda.set_device(device)
+    if world > 1:
+        import torch.distributed as td
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        td.init_process_group("nccl", device_id=device)
+    wl = workloads.make(3, nx=args.n, ny=args.n)
+    log(f"[rank {rank}] workload {wl.name}, dt={wl.dt:.6e}")
+    res = run_ours(args, wl, rank, world, device)
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        cells = wl.nx * wl.ny
+        bpc = BYTES_PER_CELL[args.dtype]
+        achieved = cells * bpc / (res["ms"] * 1e-3) / 1e9
+        traffic = ncu_traffic(args.dtype)
+        line = {
+            "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": res["ms"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[3]: {wl.nx}x{wl.ny} {args.dtype}, 6-band "
+                                   "discontinuous tensor, 3 tumour disks, h=1/64, d=10, alpha=1e-3",
+                       "kernel": res["kernel"], "l2": "working set 4.8 GB per step >> 126 MB L2",
+                       "multi_gpu": "replicas only" if world > 1 else "single GPU",
+                       "reps_ms": res["reps_ms"]},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": cells * bpc,
+                         "frac_of_nominal_8000": achieved / 8000.0},
+            "e2e": res["e2e"], "gpu_launches": res["launches"], "clocks": res["clocks"],
+        }
+        t0 = time.perf_counter()
+        line["parity_sample_max_abs_err"] = sampled_parity(wl, res["final"], args.steps)
+        log(f"sampled parity: {line['parity_sample_max_abs_err']:.3e} ({time.perf_counter() - t0:.1f} s)")
+        if not args.no_cpu and world == 1:
+            g, desc, cores, _ = oracle_sample(wl, rows=1024, steps=20)
+            line["cpu_baseline"] = {"value": g, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": desc}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        td.barrier()
+        td.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -164,6 +164,10 @@ def gg_destroy(ctx):
     _check(None, load().gg_destroy(ctx))
 
 
+def gg_last_error(ctx=None) -> str:
+    return (load().gg_last_error(ctx) or b"").decode()
+
+
 def gg_version() -> str:
     return load().gg_version().decode()
 

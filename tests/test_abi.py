@@ -1,0 +1,127 @@
+"""CPU-tier checks of the boundary: libgg.so builds, loads without a GPU, exports every symbol
+include/gg.h declares, the binding covers the same set, and host-side argument validation works.
+No compute call is made here (those need a device and live in test_gpu_parity.py)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_2006_01748_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "gg.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gg_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_declares_the_north_star_calls():
+    names = declared_symbols()
+    for need in ("gg_create", "gg_set_tensor", "gg_set_state", "gg_step", "gg_get_state"):
+        assert need in names
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    path = build.build()
+    assert os.path.exists(path)
+    lib = ctypes.CDLL(path)
+    for name in declared_symbols():
+        assert hasattr(lib, name), f"libgg.so does not export {name}"
+
+
+def test_binding_covers_exactly_the_header():
+    assert sorted(binding.SIGNATURES) == declared_symbols()
+    for name in binding.SIGNATURES:
+        assert callable(getattr(binding, name)), f"binding lacks a function named {name}"
+
+
+def test_library_has_sm100a_code_and_tma():
+    """The shipped cubin is for sm_100a and the stream kernel really uses TMA (UTMALDG in SASS)."""
+    import subprocess
+    cuobjdump = "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    out = subprocess.run([cuobjdump, "-lelf", build.build()], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    sass = subprocess.run([cuobjdump, "-sass", "-fun",
+                           "_ZN2gg14gg_step_streamIdLi2ELi3ELi10EEEvNS_10StreamArgsE", build.LIB],
+                          capture_output=True, text=True).stdout
+    assert "UTMALDG" in sass
+    assert "DFMA" in sass
+
+
+def test_create_validates_arguments():
+    ok = binding.gg_create(8, 6, 0.5, 1.0, 10.0, 1e-3, 1.0)
+    assert binding.gg_workspace_bytes(ok) >= 9 * 8 * 6 * 8
+    binding.gg_destroy(ok)
+    bad = [
+        dict(nx=1, ny=8), dict(nx=8, ny=1), dict(h=0.0), dict(h=-1.0), dict(h=float("nan")),
+        dict(dtype=7), dict(r=float("inf")),
+    ]
+    for kw in bad:
+        args = dict(nx=8, ny=8, h=0.5, r=1.0, d=10.0, alpha=1e-3, c=1.0, dtype=binding.GG_F64)
+        args.update(kw)
+        with pytest.raises(binding.GGError) as e:
+            binding.gg_create(**args)
+        assert e.value.code in (binding.GG_ERR_ARG, binding.GG_ERR_UNSUPPORTED)
+        assert str(e.value)
+
+
+def test_calls_before_bind_are_state_errors():
+    ctx = binding.gg_create(8, 8, 0.5, 1.0, 10.0, 1e-3, 1.0)
+    try:
+        with pytest.raises(binding.GGError) as e:
+            binding.gg_step(ctx, 1, 1e-3)
+        assert e.value.code == binding.GG_ERR_STATE
+        with pytest.raises(binding.GGError) as e:
+            binding.gg_set_state(ctx, 1, 1, 1)
+        assert e.value.code == binding.GG_ERR_STATE
+        with pytest.raises(binding.GGError) as e:
+            binding.gg_bind(ctx, 0, 1 << 20, 0)
+        assert e.value.code == binding.GG_ERR_ARG
+        assert binding.gg_last_step_ms(ctx) < 0
+        assert binding.gg_launches(ctx) == 0
+    finally:
+        binding.gg_destroy(ctx)
+
+
+def test_options_validate():
+    ctx = binding.gg_create(10, 8, 0.5, 1.0, 10.0, 1e-3, 1.0, binding.GG_F32)  # 40-byte rows
+    try:
+        assert binding.gg_kernel_used(ctx) == binding.GG_KERNEL_GENERIC  # AUTO: TMA needs 16 B rows
+        with pytest.raises(binding.GGError) as e:
+            binding.gg_set_option(ctx, binding.GG_OPT_KERNEL, binding.GG_KERNEL_STREAM)
+        assert e.value.code == binding.GG_ERR_UNSUPPORTED
+        with pytest.raises(binding.GGError):
+            binding.gg_set_option(ctx, 99, 0)
+        with pytest.raises(binding.GGError):
+            binding.gg_set_option(ctx, binding.GG_OPT_STREAM_VARIANT, binding.gg_num_stream_variants())
+        binding.gg_set_option(ctx, binding.GG_OPT_GRAPH, 0)
+    finally:
+        binding.gg_destroy(ctx)
+    ctx = binding.gg_create(12, 8, 0.5, 1.0, 10.0, 1e-3, 1.0, binding.GG_F32)
+    try:
+        assert binding.gg_kernel_used(ctx) == binding.GG_KERNEL_STREAM
+    finally:
+        binding.gg_destroy(ctx)
+
+
+def test_no_cpu_fallback_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("device present")
+    with pytest.raises(RuntimeError):
+        binding.Simulation(8, 8, 0.5, 1.0, 10.0, 1e-3, 1.0)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2006_01748_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
+                assert "gg_oracle" not in text, f

@@ -1,0 +1,225 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle,
+element by element on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): fp64 max-abs 1e-10 per field, fp32
+storage 2e-4, after the stated step count.  The oracle always runs in fp64 from the fp64 inputs;
+the fp32 GPU path gets the same arrays rounded to nearest fp32 (reading A10).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2006_01748_b200 import binding, workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-10, "f32": 2e-4}
+KERNELS = {"generic": binding.GG_KERNEL_GENERIC, "stream": binding.GG_KERNEL_STREAM}
+
+
+def oracle_run(wl, steps):
+    outs = [oracle.step(wl.U[s], wl.V[s], wl.W[s], wl.a, wl.b, wl.c, r=wl.r[s], d=wl.d[s],
+                        alpha=wl.alpha[s], c_r=wl.c_r[s], n=steps, dt=wl.dt, dx=wl.h)
+            for s in range(wl.batch)]
+    return tuple(np.stack([o[f] for o in outs]) for f in range(3))
+
+
+def gpu_run(wl, steps, dtype="f64", kernel=None, options=(), split=None):
+    with binding.from_workload(wl, dtype=dtype) as sim:
+        if kernel is not None:
+            sim.set_option(binding.GG_OPT_KERNEL, KERNELS[kernel])
+        for opt, val in options:
+            sim.set_option(opt, val)
+        for n in (split or [steps]):
+            sim.step(n, wl.dt)
+        used = sim.kernel
+        launches = sim.launches
+        out = sim.get_state_numpy()
+    assert launches == steps
+    return out, used
+
+
+def assert_close(got, ref, dtype, what=""):
+    for name, g, r in zip("UVW", got, ref):
+        assert g.shape == r.shape
+        assert np.isfinite(g).all(), f"{what}: non-finite {name}"
+        err = float(np.max(np.abs(g.astype(np.float64) - r)))
+        assert err <= TOL[dtype], f"{what}: field {name} max-abs error {err:.3e} > {TOL[dtype]:.0e}"
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs (0 and 1 at full size and step count; 2-4 at oracle-sized grids with the
+# same recipe, ragged in both directions so that strips, chunks and TMA boxes have partial tails)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", ["stream", "generic"])
+def test_config0_full(kernel):
+    wl = workloads.make(0)
+    got, used = gpu_run(wl, wl.steps, kernel=kernel)
+    assert used == kernel
+    assert_close(got, oracle_run(wl, wl.steps), "f64", f"cfg0 {kernel}")
+
+
+def test_config1_full():
+    wl = workloads.make(1)
+    got, used = gpu_run(wl, wl.steps)
+    assert used == "stream"
+    ref = oracle_run(wl, wl.steps)
+    assert_close(got, ref, "f64", "cfg1")
+
+
+def test_config1_undershoot_is_reproduced_not_repaired():
+    """Reading A7: with b != 0 the scheme drives W slightly below 0 (and then U above 1) early in
+    the run; the GPU must show the same values as the oracle, never a clamped field."""
+    wl = workloads.make(1)
+    got, _ = gpu_run(wl, 6)
+    ref = oracle_run(wl, 6)
+    assert ref[2].min() < -1e-5 and ref[0].max() > 1.0
+    assert got[2].min() < -1e-5 and got[0].max() > 1.0
+    assert_close(got, ref, "f64", "cfg1 after 6 steps")
+
+
+@pytest.mark.parametrize("d", [2.0, 10.0, 20.0])
+def test_config2_reduced_d_sweep(d):
+    wl = workloads.make(2, nx=328, ny=203, steps=400, d=d)
+    got, _ = gpu_run(wl, wl.steps)
+    assert_close(got, oracle_run(wl, wl.steps), "f64", f"cfg2 d={d}")
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("kernel", ["stream", "generic"])
+def test_config3_reduced_banded(dtype, kernel):
+    wl = workloads.make(3, nx=392, ny=250, steps=300)
+    got, _ = gpu_run(wl, wl.steps, dtype=dtype, kernel=kernel)
+    assert_close(got, oracle_run(wl, wl.steps), dtype, f"cfg3 {dtype} {kernel}")
+
+
+def test_config4_reduced_batch():
+    wl = workloads.make(4, nx=136, ny=90, batch=6, steps=250)
+    assert len(set(wl.d)) > 1 and len(set(wl.alpha)) > 1
+    got, _ = gpu_run(wl, wl.steps)
+    assert_close(got, oracle_run(wl, wl.steps), "f64", "cfg4")
+
+
+# ---------------------------------------------------------------------------------------------
+# random problems on awkward shapes, every kernel and every tuned build of the stream kernel
+# ---------------------------------------------------------------------------------------------
+SHAPES = [(2, 2), (2, 7), (4, 2), (64, 5), (66, 37), (130, 3), (258, 71), (62, 129)]
+
+
+@pytest.mark.parametrize("nx,ny", SHAPES)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_random_shapes(nx, ny, dtype):
+    wl = workloads.random_problem(nx * 1000 + ny, nx, ny)
+    ref = oracle_run(wl, 9)
+    kernels = ["generic"]
+    if (nx * (8 if dtype == "f64" else 4)) % 16 == 0:
+        kernels.append("stream")
+    for kernel in kernels:
+        got, used = gpu_run(wl, 9, dtype=dtype, kernel=kernel)
+        assert used == kernel
+        assert_close(got, ref, dtype, f"{nx}x{ny} {dtype} {kernel}")
+
+
+@pytest.mark.parametrize("nx,ny", [(65, 9), (3, 3), (127, 33)])
+def test_odd_width_takes_generic_path(nx, ny):
+    wl = workloads.random_problem(7 + nx, nx, ny)
+    got, used = gpu_run(wl, 5)
+    assert used == "generic"  # AUTO never mis-computes: rows are not 16-byte multiples
+    assert_close(got, oracle_run(wl, 5), "f64", f"{nx}x{ny}")
+
+
+def test_every_stream_variant_and_chunking():
+    wl = workloads.random_problem(42, 200, 150, batch=2)
+    ref = oracle_run(wl, 7)
+    for v in range(binding.gg_num_stream_variants()):
+        for ipw in (1, 4, 64):
+            got, _ = gpu_run(wl, 7, kernel="stream",
+                             options=[(binding.GG_OPT_STREAM_VARIANT, v),
+                                      (binding.GG_OPT_ITEMS_PER_WARP, ipw)])
+            assert_close(got, ref, "f64", f"variant {v} items/warp {ipw}")
+
+
+def test_stream_and_generic_agree_closely():
+    """Two independent kernels inside the library: same scheme, different evaluation order."""
+    wl = workloads.random_problem(5, 192, 96)
+    a, _ = gpu_run(wl, 50, kernel="stream")
+    b, _ = gpu_run(wl, 50, kernel="generic")
+    for x, y in zip(a, b):
+        assert np.max(np.abs(x - y)) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# step loop: graphs, ping-pong parity, repeated calls
+# ---------------------------------------------------------------------------------------------
+def test_graph_and_plain_launches_give_identical_bits():
+    wl = workloads.make(0)
+    a, _ = gpu_run(wl, 131, options=[(binding.GG_OPT_GRAPH, 1), (binding.GG_OPT_GRAPH_CHUNK, 16)])
+    b, _ = gpu_run(wl, 131, options=[(binding.GG_OPT_GRAPH, 0)])
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_split_calls_equal_one_call():
+    wl = workloads.make(1, nx=128, ny=96)
+    a, _ = gpu_run(wl, 37)
+    b, _ = gpu_run(wl, 37, split=[1, 0, 3, 20, 13])
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    assert_close(a, oracle_run(wl, 37), "f64", "split")
+
+
+def test_zero_steps_and_roundtrip():
+    wl = workloads.random_problem(3, 32, 16, batch=3)
+    with binding.from_workload(wl) as sim:
+        sim.step(0, wl.dt)
+        U, V, W = sim.get_state_numpy()
+        assert sim.launches == 0
+    assert np.array_equal(U, wl.U) and np.array_equal(V, wl.V) and np.array_equal(W, wl.W)
+
+
+def test_host_buffer_entry_points():
+    wl = workloads.random_problem(11, 96, 40)
+    with binding.Simulation(wl.nx, wl.ny, wl.h, wl.r, wl.d, wl.alpha, wl.c_r) as sim:
+        sim.set_tensor_host(wl.a, wl.b, wl.c)
+        sim.set_state_host(wl.U, wl.V, wl.W)
+        sim.step(6, wl.dt)
+        out = [np.empty_like(wl.U) for _ in range(3)]
+        sim.get_state_host(*out)
+        assert sim.last_step_ms() >= 0.0
+    assert_close(out, oracle_run(wl, 6), "f64", "host entry points")
+
+
+def test_errors_on_device():
+    wl = workloads.random_problem(1, 16, 8)
+    with binding.from_workload(wl) as sim:
+        for bad in (0.0, -1.0, float("nan"), float("inf")):
+            with pytest.raises(binding.GGError) as e:
+                sim.step(1, bad)
+            assert e.value.code == binding.GG_ERR_ARG
+        with pytest.raises(binding.GGError):
+            sim.step(-1, wl.dt)
+    with binding.Simulation(16, 8, wl.h, 1, 1, 1, 1) as sim:
+        with pytest.raises(binding.GGError) as e:
+            sim.step(1, wl.dt)  # no tensor / state yet
+        assert e.value.code == binding.GG_ERR_STATE
+
+
+# ---------------------------------------------------------------------------------------------
+# physics invariants on the GPU result itself (hold at any size)
+# ---------------------------------------------------------------------------------------------
+def test_equilibria_and_uniform_data_on_gpu():
+    wl = workloads.random_problem(8, 128, 64)
+    one, zero = np.ones_like(wl.U), np.zeros_like(wl.U)
+    for (u, v, w) in [(one, zero, zero), (zero, one, one), (zero, zero, zero)]:
+        wl.U, wl.V, wl.W = u, v, w
+        got, _ = gpu_run(wl, 20)
+        assert np.array_equal(got[0], u) and np.array_equal(got[1], v) and np.array_equal(got[2], w)
+
+
+def test_mass_conservation_on_gpu():
+    wl = workloads.random_problem(9, 256, 128)
+    wl.c_r[:] = 0.0
+    wl.r[:] = 0.0
+    got, _ = gpu_run(wl, 200)
+    assert abs(got[2].sum() - wl.W.sum()) <= 1e-12 * wl.W.sum()
+    assert abs(got[1].sum() - wl.V.sum()) <= 1e-12 * wl.V.sum()
