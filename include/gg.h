@@ -76,7 +76,8 @@ enum {
     GG_OPT_GRAPH_CHUNK = 2, /* steps per captured graph (default 64)                            */
     GG_OPT_STREAM_VARIANT = 3,  /* tuning: which (rows/box, stages, warps/CTA) build of the STREAM
                                    kernel runs; 0 .. gg_num_stream_variants()-1                  */
-    GG_OPT_ITEMS_PER_WARP = 4   /* tuning: target work items (row chunk x strip) per resident warp */
+    GG_OPT_ITEMS_PER_WARP = 4,  /* tuning: target work items (row chunk x tile column) per resident CTA */
+    GG_OPT_STREAM_WARPS = 5     /* tuning: warps (= 512-byte strips) per CTA: 1, 2, 4, 8; 0 = from nx */
 };
 
 /* One simulation.  nx, ny >= 2 cells; h > 0 the mesh size (dx = dy = h);

@@ -21,7 +21,8 @@ from . import build as _build
 GG_F64, GG_F32 = 0, 1
 GG_OK, GG_ERR_ARG, GG_ERR_STATE, GG_ERR_CUDA, GG_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
 GG_KERNEL_AUTO, GG_KERNEL_GENERIC, GG_KERNEL_STREAM, GG_KERNEL_STREAM2, GG_KERNEL_RESIDENT = range(5)
-GG_OPT_KERNEL, GG_OPT_GRAPH, GG_OPT_GRAPH_CHUNK, GG_OPT_STREAM_VARIANT, GG_OPT_ITEMS_PER_WARP = range(5)
+GG_OPT_KERNEL, GG_OPT_GRAPH, GG_OPT_GRAPH_CHUNK, GG_OPT_STREAM_VARIANT, GG_OPT_ITEMS_PER_WARP, \
+    GG_OPT_STREAM_WARPS = range(6)
 
 KERNEL_NAMES = {GG_KERNEL_AUTO: "auto", GG_KERNEL_GENERIC: "generic", GG_KERNEL_STREAM: "stream",
                 GG_KERNEL_STREAM2: "stream2", GG_KERNEL_RESIDENT: "resident"}

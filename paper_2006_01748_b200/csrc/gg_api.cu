@@ -57,7 +57,8 @@ struct gg_ctx {
     int opt_graph = 1;
     long long opt_chunk = 64;
     int opt_variant = 0;
-    int opt_items_per_warp = 4;
+    int opt_items_per_warp = 4;   // work items per resident CTA
+    int opt_warps = 0;            // warps (strips) per CTA; 0 = from the grid width
     // stream-kernel plan (tensor maps etc.)
     gg::StreamPlan plan;
     bool plan_ready = false;
@@ -131,24 +132,35 @@ void drop_graphs(gg_ctx* c) {
 // ------------------------------------------------------------------------------------------
 namespace {
 
-// Stream kernel instantiations (rows per TMA box, ring stages per warp, warps per CTA); the
-// default is the one tuned on B200, the others stay selectable through
+// Stream kernel instantiations: tuning index v = (rows per TMA box RB, ring stages NST), crossed
+// with the warps (= strips) per CTA, NW in {1, 2, 4, 8}, which the plan picks from the grid width.
+// v = 0 is the build tuned on B200; the others stay selectable through
 // GG_OPT_STREAM_VARIANT for re-tuning.
-struct Variant { int rb, nst, nw; };
-constexpr Variant kVariants[] = {{2, 3, 10}, {2, 2, 16}, {4, 2, 8}, {2, 4, 8}, {1, 3, 16}, {1, 4, 12}};
+struct Variant { int rb, nst; };
+constexpr Variant kVariants[] = {{2, 4}, {4, 2}, {2, 3}, {1, 6}, {1, 8}, {4, 3}};
 constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
-constexpr int kDefaultVariant = 0;
+constexpr int kDefaultVariant = 1;
 
-// Calls F.template operator()<T, RB, NST, NW>() for variant v.
+template <typename T, int RB, int NST, typename F>
+int with_nw(int nw, F&& f) {
+    switch (nw) {
+        case 1: return f.template operator()<T, RB, NST, 1>();
+        case 2: return f.template operator()<T, RB, NST, 2>();
+        case 4: return f.template operator()<T, RB, NST, 4>();
+        case 8: return f.template operator()<T, RB, NST, 8>();
+    }
+    return -1;
+}
+// Calls f.template operator()<T, RB, NST, NW>() for tuning index v and nw warps per CTA.
 template <typename T, typename F>
-int with_variant(int v, F&& f) {
+int with_variant(int v, int nw, F&& f) {
     switch (v) {
-        case 0: return f.template operator()<T, 2, 3, 10>();
-        case 1: return f.template operator()<T, 2, 2, 16>();
-        case 2: return f.template operator()<T, 4, 2, 8>();
-        case 3: return f.template operator()<T, 2, 4, 8>();
-        case 4: return f.template operator()<T, 1, 3, 16>();
-        case 5: return f.template operator()<T, 1, 4, 12>();
+        case 0: return with_nw<T, 2, 4>(nw, f);
+        case 1: return with_nw<T, 4, 2>(nw, f);
+        case 2: return with_nw<T, 2, 3>(nw, f);
+        case 3: return with_nw<T, 1, 6>(nw, f);
+        case 4: return with_nw<T, 1, 8>(nw, f);
+        case 5: return nw <= 4 ? with_nw<T, 4, 3>(nw, f) : -1;  // 8 warps would not fit in smem
     }
     return -1;
 }
@@ -170,13 +182,13 @@ EncodeTiledFn encode_fn() {
     return fn;
 }
 
-int make_map(gg_ctx* c, CUtensorMap* m, void* base, int depth, int box_rows) {
+int make_map(gg_ctx* c, CUtensorMap* m, void* base, int depth, int box_bytes, int box_rows) {
     EncodeTiledFn enc = encode_fn();
     if (!enc) return fail(c, GG_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
     const size_t es = c->esize();
     cuuint64_t dims[3] = {(cuuint64_t)c->nx, (cuuint64_t)c->ny, (cuuint64_t)depth};
     cuuint64_t strides[2] = {(cuuint64_t)c->nx * es, (cuuint64_t)c->plane() * es};
-    cuuint32_t box[3] = {(cuuint32_t)(gg::kRowBytes / es), (cuuint32_t)box_rows, 1};
+    cuuint32_t box[3] = {(cuuint32_t)(box_bytes / es), (cuuint32_t)box_rows, 1};
     cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = enc(m, c->dtype == GG_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64
                                            : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
@@ -209,40 +221,50 @@ int build_plan(gg_ctx* c) {
         return fail(c, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0");
     gg::StreamPlan& P = c->plan;
     const Variant var = kVariants[c->opt_variant];
-    const int kRB = var.rb, kNST = var.nst, kNW = var.nw;
+    const int strip_cells = gg::kStripBytes / (int)c->esize();
+    const int nstrips = (c->nx + strip_cells - 1) / strip_cells;
+    int nw = c->opt_warps;
+    if (nw == 0) nw = nstrips >= 8 ? 8 : nstrips >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
+    if (c->opt_variant == 5 && nw > 4) nw = 4;
+    P.rb = var.rb; P.nst = var.nst; P.nw = nw;
     for (int p = 0; p < 2; ++p)
         for (int f = 0; f < 3; ++f) {
-            int rc = make_map(c, &P.state[p][f], c->state[p][f], c->nbatch, kRB);
+            int rc = make_map(c, &P.state[p][f], c->state[p][f], c->nbatch, gg::kStripBytes, P.rb);
+            if (rc) return rc;
+            rc = make_map(c, &P.state_halo[p][f], c->state[p][f], c->nbatch, gg::kHaloBytes, P.rb);
             if (rc) return rc;
         }
     for (int f = 0; f < 3; ++f) {
-        int rc = make_map(c, &P.coef[f], c->coef[f], 1, kRB);
+        int rc = make_map(c, &P.coef[f], c->coef[f], 1, gg::kStripBytes, P.rb);
         if (rc) return rc;
+        if (f < 2) {
+            rc = make_map(c, &P.coef_halo[f], c->coef[f], 1, gg::kHaloBytes, P.rb);
+            if (rc) return rc;
+        }
     }
-    const int strip_cells = gg::kStripBytes / (int)c->esize();
-    P.nstrips = (c->nx + strip_cells - 1) / strip_cells;
-    P.rb = kRB; P.nst = kNST; P.nw = kNW;
-    P.block = kNW * 32;
-    P.smem = (size_t)((kNW * kNST * 8 + 127) / 128 * 128) +
-             (size_t)kNW * kNST * 6 * ((kRB * gg::kRowBytes + 127) / 128 * 128);
+    P.block = nw * 32;
+    P.smem = (size_t)gg::stream_smem_bytes(P.rb, P.nst, nw);
     const void* fn = nullptr;
-    if (c->dtype == GG_F64) with_variant<double>(c->opt_variant, KernelPtr{&fn});
-    else with_variant<float>(c->opt_variant, KernelPtr{&fn});
+    int rc = c->dtype == GG_F64 ? with_variant<double>(c->opt_variant, nw, KernelPtr{&fn})
+                                : with_variant<float>(c->opt_variant, nw, KernelPtr{&fn});
+    if (rc || !fn) return fail(c, GG_ERR_UNSUPPORTED, "no stream kernel build for variant %d, %d warps", c->opt_variant, nw);
     GG_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem));
-    // Row chunks: enough items that every warp of a full grid gets several, none shorter than
-    // 16 rows (the two halo rows per chunk are re-read, from L2 when neighbours run together).
-    const long long warps = (long long)c->num_sms * kNW;
-    long long want = (long long)c->opt_items_per_warp * warps;  // target items
-    long long per = (long long)P.nstrips * c->nbatch;
-    long long nchunks = (want + per - 1) / per;
-    long long max_chunks = (c->ny + 15) / 16;
+    int per_sm = 0;
+    GG_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, P.block, P.smem));
+    if (per_sm < 1) return fail(c, GG_ERR_CUDA, "stream kernel does not fit on an SM");
+    const long long resident = (long long)c->num_sms * per_sm;
+    // Row chunks: about opt_items_per_cta items per resident CTA (static round-robin schedule),
+    // none shorter than 16 rows (each chunk re-reads two halo rows and recomputes one).
+    P.ntilecols = (nstrips + nw - 1) / nw;
+    const long long per = (long long)P.ntilecols * c->nbatch;
+    long long nchunks = ((long long)c->opt_items_per_warp * resident + per - 1) / per;
+    const long long max_chunks = (c->ny + 15) / 16;
     if (nchunks > max_chunks) nchunks = max_chunks;
     if (nchunks < 1) nchunks = 1;
     P.chunk_rows = (int)((c->ny + nchunks - 1) / nchunks);
     P.nchunks = (c->ny + P.chunk_rows - 1) / P.chunk_rows;
-    P.nitems = (long long)P.nstrips * P.nchunks * c->nbatch;
-    long long ctas = (P.nitems + kNW - 1) / kNW;
-    P.grid = (int)(ctas < c->num_sms ? ctas : c->num_sms);
+    P.nitems = (long long)P.ntilecols * P.nchunks * c->nbatch;
+    P.grid = (int)(P.nitems < resident ? P.nitems : resident);
     c->plan_ready = true;
     return GG_OK;
 }
@@ -268,14 +290,16 @@ int launch_stream(gg_ctx* c, int src, double dt) {
     gg::StreamArgs a;
     a.mU = P.state[src][0]; a.mV = P.state[src][1]; a.mW = P.state[src][2];
     a.ma = P.coef[0]; a.mb = P.coef[1]; a.mc = P.coef[2];
+    a.hU = P.state_halo[src][0]; a.hV = P.state_halo[src][1]; a.hW = P.state_halo[src][2];
+    a.ha = P.coef_halo[0]; a.hb = P.coef_halo[1];
     a.U1 = c->state[src ^ 1][0]; a.V1 = c->state[src ^ 1][1]; a.W1 = c->state[src ^ 1][2];
     a.sims = c->d_sims;
     a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
-    a.nstrips = P.nstrips; a.nchunks = P.nchunks; a.chunk_rows = P.chunk_rows;
+    a.ntilecols = P.ntilecols; a.nchunks = P.nchunks; a.chunk_rows = P.chunk_rows;
     a.nitems = P.nitems;
     a.dt = dt; a.inv_h2 = 1.0 / (c->h * c->h);
-    if (c->dtype == GG_F64) with_variant<double>(c->opt_variant, KernelLaunch{&P, &a, c->stream});
-    else with_variant<float>(c->opt_variant, KernelLaunch{&P, &a, c->stream});
+    if (c->dtype == GG_F64) with_variant<double>(c->opt_variant, P.nw, KernelLaunch{&P, &a, c->stream});
+    else with_variant<float>(c->opt_variant, P.nw, KernelLaunch{&P, &a, c->stream});
     GG_CUDA(c, cudaGetLastError());
     return GG_OK;
 }
@@ -506,7 +530,11 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
             if (value < 0 || value >= kNumVariants) return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_VARIANT: 0..%d", kNumVariants - 1);
             break;
         case GG_OPT_ITEMS_PER_WARP:
-            if (value < 1 || value > 1024) return fail(ctx, GG_ERR_ARG, "GG_OPT_ITEMS_PER_WARP: 1..1024");
+            if (value < 1 || value > 1024) return fail(ctx, GG_ERR_ARG, "GG_OPT_ITEMS_PER_CTA: 1..1024");
+            break;
+        case GG_OPT_STREAM_WARPS:
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8)
+                return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_WARPS: 0, 1, 2, 4 or 8");
             break;
         default:
             return fail(ctx, GG_ERR_UNSUPPORTED, "gg_set_option: unknown option %d", option);
@@ -518,6 +546,7 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
         case GG_OPT_GRAPH_CHUNK: ctx->opt_chunk = value; break;
         case GG_OPT_STREAM_VARIANT: ctx->opt_variant = (int)value; ctx->plan_ready = false; break;
         case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = false; break;
+        case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = false; break;
     }
     return GG_OK;
 }

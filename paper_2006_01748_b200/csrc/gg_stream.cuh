@@ -1,60 +1,77 @@
 // gg_stream.cuh -- GG_KERNEL_STREAM: the fused single-step kernel for sm_100a.
 //
 // Design.  The step is HBM-bound (72 B and ~45 flops per cell in fp64), so
-// the kernel is built around keeping many TMA loads in flight and touching every byte once:
+// the kernel is built around keeping many TMA loads in flight and touching every DRAM byte once:
 //
-//  * The grid is cut into column STRIPS 512 bytes wide (64 fp64 / 128 fp32 cells) and row CHUNKS.
-//    One WARP owns one (simulation, chunk, strip) item at a time and is a self-contained
-//    producer + consumer: its lane 0 issues `cp.async.bulk.tensor` (TMA) loads of RB-row boxes of
-//    the six input arrays (U, V, W, a, b, c; strip plus a 16-byte halo on each side, rows j0-1..j1)
-//    into a warp-private ring of NST stages in shared memory, completion signalled on one
-//    mbarrier per stage.  No __syncthreads, no inter-warp dependence: warps drift apart and keep
-//    the memory system evenly loaded.  Out-of-domain parts of a box are zero-filled by TMA.
-//  * The warp marches up its strip one row at a time.  Every lane owns 16 bytes of each row
-//    (2 fp64 / 4 fp32 cells) and keeps a rolling window of rows j-1, j, j+1 in REGISTERS, so each
-//    shared-memory element is read once per lane that needs it.  The north face fluxes of row j
-//    are kept and reused as the south face fluxes of row j+1; x-face fluxes inside a lane's run
-//    are computed once and used by both adjacent cells.  (The run's west face is recomputed by
-//    the lane instead of shuffled from its neighbour: cheaper than the exchange.)
+//  * The grid is cut into TILE COLUMNS of NW adjacent STRIPS, each strip 512 bytes wide (64 fp64 /
+//    128 fp32 cells), and into row CHUNKS.  One CTA of NW warps owns one (simulation, chunk, tile
+//    column) item at a time; warp w owns strip w of the tile and marches up it row by row.
+//  * Input rows travel through an NST-stage ring in shared memory, RB rows per stage.  Every warp
+//    is the producer of its own strip: its lane 0 issues `cp.async.bulk.tensor` (TMA) loads of
+//    exactly aligned RB x 512-byte boxes of the six input arrays (U, V, W, a, b, c) -- whole
+//    32-byte sectors and 128-byte lines only, so nothing is fetched from L2/DRAM twice.  The one
+//    column of halo each side of the TILE comes from two 16-byte-wide boxes per array; inside the
+//    tile a strip's halo column is simply its neighbour warp's edge column in shared memory.
+//    (A first version gave every warp its own 544-byte box with the halo inside: ncu showed
+//    1.34x the compulsory DRAM reads, because TMA fetches whole 128-byte lines at both ragged
+//    ends and independent warps drift too far apart for L2 to merge them.)
+//    One `full` mbarrier per stage (NW producer arrivals + the bytes) and one `empty` mbarrier
+//    (NW consumer arrivals); no __syncthreads anywhere.  Out-of-domain box parts are zero-filled.
+//  * Every lane owns 16 bytes of each row (2 fp64 / 4 fp32 cells) and keeps a rolling window of
+//    rows j-1, j, j+1 in REGISTERS, so each shared-memory element is read once per lane that needs
+//    it.  The north face fluxes of row j are kept and reused as the south face fluxes of row j+1;
+//    x-face fluxes inside a lane's run are computed once and used by both adjacent cells.  (The
+//    run's west face is recomputed by the lane instead of shuffled from its neighbour: same cost
+//    as the exchange plus its divergent edge case, and no cross-lane dependence.)
 //  * Neumann boundaries (reading A2): faces on the domain boundary carry zero flux, tangential
 //    differences use the mirrored neighbour.  Handled with warp-uniform row tests and two
 //    per-lane flags; TMA's zero fill keeps every discarded value finite.
-//  * Results leave as one 16-byte store per lane per field per row: 512 contiguous bytes per warp.
+//  * Results leave as one 16-byte store per lane per field per row: 512 contiguous bytes per warp,
+//    NW x 512 contiguous bytes per CTA row.
 #pragma once
 #include <cuda.h>
+
+#include <type_traits>
 
 #include "gg_common.cuh"
 
 namespace gg {
 
-constexpr int kStripBytes = 512;              // 32 lanes x 16 B
-constexpr int kRowBytes = kStripBytes + 32;   // + 16 B halo each side (TMA box inner extent)
-
-template <int RB>
-__host__ __device__ constexpr int slab_bytes() { return (RB * kRowBytes + 127) / 128 * 128; }
+constexpr int kStripBytes = 512;   // 32 lanes x 16 B
+constexpr int kHaloBytes = 16;     // inner extent of a tile-edge halo box (minimum TMA box width)
+constexpr int kHaloSlab = 128;     // shared-memory bytes reserved per halo box (TMA dst alignment)
 
 struct alignas(64) StreamArgs {
-    CUtensorMap mU, mV, mW, ma, mb, mc;  // rank-3 maps {nx, ny, B}, box {row, RB, 1}
+    // rank-3 tensor maps {nx, ny, B}: main boxes {512 B, RB, 1}; halo boxes {16 B, RB, 1}
+    CUtensorMap mU, mV, mW, ma, mb, mc;
+    CUtensorMap hU, hV, hW, ha, hb;
     void* U1;                            // outputs [B][ny][nx]
     void* V1;
     void* W1;
     const SimScalars* sims;
     int nx, ny, nbatch;
-    int nstrips, nchunks, chunk_rows;
+    int ntilecols, nchunks, chunk_rows;
     long long nitems;
     double dt, inv_h2;
 };
 
 // Host-side plan: tensor maps for both ping-pong copies and the launch geometry.
 struct StreamPlan {
-    CUtensorMap state[2][3];
-    CUtensorMap coef[3];
-    int nstrips = 0, nchunks = 0, chunk_rows = 0;
+    CUtensorMap state[2][3], state_halo[2][3];
+    CUtensorMap coef[3], coef_halo[2];
+    int ntilecols = 0, nchunks = 0, chunk_rows = 0;
     long long nitems = 0;
     int grid = 0, block = 0;
     size_t smem = 0;
     int rb = 0, nst = 0, nw = 0;
 };
+
+__host__ __device__ constexpr int stream_stage_bytes(int rb, int nw) {
+    return nw * 6 * rb * kStripBytes + 2 * 5 * kHaloSlab;
+}
+__host__ __device__ constexpr int stream_smem_bytes(int rb, int nst, int nw) {
+    return 128 + nst * stream_stage_bytes(rb, nw);
+}
 
 // ------------------------------------------------------------------------------------------
 // PTX wrappers (sm_100a)
@@ -126,74 +143,138 @@ __device__ __forceinline__ void stg_own(T* g, const T* x) {
     *reinterpret_cast<typename Vec16<T>::type*>(g) = v;
 }
 
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// own C cells from `own`, west / east neighbour elements from wherever they live
+template <typename T, int C>
+__device__ __forceinline__ void lds_run(const char* own, const char* west, const char* east, T* x) {
+    lds_own<T, C>(own, x + 1);
+    x[0] = *reinterpret_cast<const T*>(west);
+    x[C + 1] = *reinterpret_cast<const T*>(east);
+}
+
+// One work item of a CTA: simulation `sim`, tile column starting at cell i0, rows [j0, j1).
+struct StreamItem {
+    int sim, i0, j0, j1, nr, nstage;
+};
+template <int RB, int TILE_CELLS>
+__device__ __forceinline__ StreamItem stream_item(const StreamArgs& A, long long item) {
+    StreamItem it;
+    const int tc = (int)(item % A.ntilecols);
+    const long long t = item / A.ntilecols;
+    const int chunk = (int)(t % A.nchunks);
+    it.sim = (int)(t / A.nchunks);
+    it.i0 = tc * TILE_CELLS;
+    it.j0 = chunk * A.chunk_rows;
+    it.j1 = min(it.j0 + A.chunk_rows, A.ny);
+    it.nr = it.j1 - it.j0 + 2;  // input rows j0-1 .. j1 arrive
+    it.nstage = (it.nr + RB - 1) / RB;
+    return it;
+}
+
 // ------------------------------------------------------------------------------------------
 // The kernel.  T: arithmetic/storage type; RB: rows per TMA box (= per ring stage); NST: ring
-// stages per warp; NW: warps per CTA.  Dynamic shared memory:
-//   [NW*NST mbarriers, padded to 128 B][NW warps][NST stages][6 arrays][slab_bytes<RB>()]
+// stages; NW: warps (= strips) per CTA.  Dynamic shared memory:
+//   [full[NST], empty[NST] mbarriers, 128 B][NST stages]; a stage is
+//   [NW warps][6 arrays][RB rows][512 B] followed by [west, east][5 arrays][128 B halo slab].
 // ------------------------------------------------------------------------------------------
 template <typename T, int RB, int NST, int NW>
 __global__ void __launch_bounds__(NW * 32, 1) gg_step_stream(const __grid_constant__ StreamArgs A) {
     constexpr int C = 16 / (int)sizeof(T);  // cells per lane per row
     constexpr int SW = 32 * C;              // strip width in cells
     constexpr int E = C + 2;                // extended run: west nbr, C own cells, east nbr
-    constexpr int SLAB = slab_bytes<RB>();
-    constexpr int STAGE = 6 * SLAB;
-    constexpr uint32_t STAGE_TX = 6u * RB * kRowBytes;
-    constexpr int BAR_BYTES = (NW * NST * 8 + 127) / 128 * 128;
+    constexpr int SLAB = RB * kStripBytes;  // one array of one warp in one stage
+    constexpr int MAIN = NW * 6 * SLAB;
+    constexpr int STAGE = stream_stage_bytes(RB, NW);
+    static_assert(RB * kHaloBytes <= kHaloSlab, "halo slab too small");
+    static_assert(2 * NST * 8 <= 128, "too many stages");
 
     extern __shared__ __align__(128) char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t bar0 = smem_u32(smem) + (uint32_t)(warp * NST) * 8u;
-    char* ring = smem + BAR_BYTES + (size_t)warp * NST * STAGE;
+    const uint32_t full0 = smem_u32(smem), empty0 = full0 + 8u * NST;
+    char* ring = smem + 128;
     const uint32_t ring_u32 = smem_u32(ring);
 
-    if (lane == 0) {
-        for (int s = 0; s < NST; ++s) mbar_init(bar0 + 8u * s, 1);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST; ++s) {
+            mbar_init(full0 + 8u * s, NW);
+            mbar_init(empty0 + 8u * s, NW);
+        }
         fence_barrier_init();
         fence_proxy_async();
     }
-    __syncwarp();
+    __syncthreads();  // once, before the pipeline starts
+
+    // per-lane byte offsets inside a stage: own run, west and east neighbour elements
+    const int ownOff = warp * 6 * SLAB + 16 * lane;
+    int wOff, wSF, wSR, eOff, eSF, eSR;  // offset, stride per array, stride per row
+    if (lane > 0) { wOff = ownOff - (int)sizeof(T); wSF = SLAB; wSR = kStripBytes; }
+    else if (warp > 0) { wOff = (warp - 1) * 6 * SLAB + kStripBytes - (int)sizeof(T); wSF = SLAB; wSR = kStripBytes; }
+    else { wOff = MAIN + kHaloBytes - (int)sizeof(T); wSF = kHaloSlab; wSR = kHaloBytes; }
+    if (lane < 31) { eOff = ownOff + 16; eSF = SLAB; eSR = kStripBytes; }
+    else if (warp < NW - 1) { eOff = (warp + 1) * 6 * SLAB; eSF = SLAB; eSR = kStripBytes; }
+    else { eOff = MAIN + 5 * kHaloSlab; eSF = kHaloSlab; eSR = kHaloBytes; }
 
     const int nx = A.nx, ny = A.ny;
     const size_t plane = (size_t)nx * ny;
-    const long long gwarp = (long long)blockIdx.x * NW + warp;
-    const long long nwarps = (long long)gridDim.x * NW;
-    uint32_t gq = 0;  // stages consumed so far by this warp (slot = gq % NST, phase = gq / NST & 1)
 
-    for (long long item = gwarp; item < A.nitems; item += nwarps) {
-        const int strip = (int)(item % A.nstrips);
-        const long long t = item / A.nstrips;
-        const int chunk = (int)(t % A.nchunks);
-        const int sim = (int)(t / A.nchunks);
-        const int i0 = strip * SW;
-        const int j0 = chunk * A.chunk_rows;
-        const int j1 = min(j0 + A.chunk_rows, ny);
-        const int nr = j1 - j0 + 2;             // rows j0-1 .. j1 arrive
-        const int nstage = (nr + RB - 1) / RB;
-        const int iown = i0 + lane * C;         // first own cell
-        const bool valid = iown < nx;           // nx % C == 0: a lane's run is all in or all out
-        const bool atW = iown == 0, atE = iown + C == nx;
-        const StepCoef<T> k = fold_coef<T>(A.sims[sim], A.dt, A.inv_h2);
-        T* gU = (T*)A.U1 + sim * plane + iown;
-        T* gV = (T*)A.V1 + sim * plane + iown;
-        T* gW = (T*)A.W1 + sim * plane + iown;
-
-        auto issue = [&](int q, uint32_t slot) {  // lane 0 only
-            const uint32_t bar = bar0 + 8u * slot;
+    // producer cursor (lane 0 of every warp issues its own strip): next global stage to issue
+    uint32_t gp = 0;
+    long long p_item = blockIdx.x;
+    int p_q = 0;
+    StreamItem pit = stream_item<RB, NW * SW>(A, p_item < A.nitems ? p_item : 0);
+    // issue global stages up to (but excluding) `limit`
+    auto produce = [&](uint32_t limit) {
+        while (gp < limit && p_item < A.nitems) {
+            const uint32_t slot = gp % NST;
+            if (gp >= NST) mbar_wait(empty0 + 8u * slot, ((gp / NST) - 1u) & 1u);
+            const uint32_t bar = full0 + 8u * slot;
             const uint32_t dst = ring_u32 + slot * STAGE;
-            const int x = i0 - C, y = j0 - 1 + q * RB;
-            mbar_expect_tx(bar, STAGE_TX);
-            tma_load_3d(dst + 0 * SLAB, &A.mU, bar, x, y, sim);
-            tma_load_3d(dst + 1 * SLAB, &A.mV, bar, x, y, sim);
-            tma_load_3d(dst + 2 * SLAB, &A.mW, bar, x, y, sim);
-            tma_load_3d(dst + 3 * SLAB, &A.ma, bar, x, y, 0);
-            tma_load_3d(dst + 4 * SLAB, &A.mb, bar, x, y, 0);
-            tma_load_3d(dst + 5 * SLAB, &A.mc, bar, x, y, 0);
-        };
-        if (lane == 0) {
-            const int pre = nstage < NST ? nstage : NST;
-            for (int q = 0; q < pre; ++q) issue(q, (gq + q) % NST);
+            const uint32_t mine = dst + warp * 6 * SLAB;
+            const int x = pit.i0 + warp * SW, y = pit.j0 - 1 + p_q * RB, z = pit.sim;
+            uint32_t bytes = 6u * SLAB;
+            if (warp == 0) bytes += 5u * RB * kHaloBytes;
+            if (warp == NW - 1) bytes += 5u * RB * kHaloBytes;
+            mbar_expect_tx(bar, bytes);
+            tma_load_3d(mine + 0 * SLAB, &A.mU, bar, x, y, z);
+            tma_load_3d(mine + 1 * SLAB, &A.mV, bar, x, y, z);
+            tma_load_3d(mine + 2 * SLAB, &A.mW, bar, x, y, z);
+            tma_load_3d(mine + 3 * SLAB, &A.ma, bar, x, y, 0);
+            tma_load_3d(mine + 4 * SLAB, &A.mb, bar, x, y, 0);
+            tma_load_3d(mine + 5 * SLAB, &A.mc, bar, x, y, 0);
+            if (warp == 0 || warp == NW - 1) {
+                for (int side = 0; side < 2; ++side) {
+                    if ((side == 0 && warp != 0) || (side == 1 && warp != NW - 1)) continue;
+                    const uint32_t h = dst + MAIN + side * 5 * kHaloSlab;
+                    const int hx = side == 0 ? pit.i0 - C : pit.i0 + NW * SW;
+                    tma_load_3d(h + 0 * kHaloSlab, &A.hU, bar, hx, y, z);
+                    tma_load_3d(h + 1 * kHaloSlab, &A.hV, bar, hx, y, z);
+                    tma_load_3d(h + 2 * kHaloSlab, &A.hW, bar, hx, y, z);
+                    tma_load_3d(h + 3 * kHaloSlab, &A.ha, bar, hx, y, 0);
+                    tma_load_3d(h + 4 * kHaloSlab, &A.hb, bar, hx, y, 0);
+                }
+            }
+            ++gp;
+            if (++p_q == pit.nstage) {
+                p_q = 0;
+                p_item += gridDim.x;
+                if (p_item < A.nitems) pit = stream_item<RB, NW * SW>(A, p_item);
+            }
         }
+    };
+
+    uint32_t gc = 0;  // global stages consumed (identical sequence in every warp of the CTA)
+    for (long long item = blockIdx.x; item < A.nitems; item += gridDim.x) {
+        const StreamItem it = stream_item<RB, NW * SW>(A, item);
+        const int j0 = it.j0, nr = it.nr;
+        const int iown = it.i0 + warp * SW + lane * C;  // first own cell
+        const bool valid = iown < nx;                   // nx % C == 0: a run is all in or all out
+        const bool atW = iown == 0, atE = iown + C == nx;
+        const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.inv_h2);
+        T* gU = (T*)A.U1 + it.sim * plane + iown;
+        T* gV = (T*)A.V1 + it.sim * plane + iown;
+        T* gW = (T*)A.W1 + it.sim * plane + iown;
 
         // rolling register window (rows jc-1, jc, jc+1 = P, C, N)
         T wP[E], wC[E], wN[E], uC[E], uN[E], vC[E], vN[E], aC[E], aN[E], bC[E], bN[E];
@@ -203,95 +284,110 @@ __global__ void __launch_bounds__(NW * 32, 1) gg_step_stream(const __grid_consta
 #pragma unroll
         for (int c = 0; c < C; ++c) cC[c] = hC[c] = sV[c] = sW[c] = (T)0;
 
-        for (int q = 0; q < nstage; ++q, ++gq) {
-            const uint32_t slot = gq % NST;
-            mbar_wait(bar0 + 8u * slot, (gq / NST) & 1u);
-            const char* st = ring + (size_t)slot * STAGE + 16 + 16 * lane;
-#pragma unroll
-            for (int rr = 0; rr < RB; ++rr) {
-                const int n = q * RB + rr;  // arrival index; arriving row = j0-1+n
-                if (n < nr) {
-                    const char* row = st + rr * kRowBytes;
-                    lds_ext<T, C>(row + 0 * SLAB, uN);
-                    lds_ext<T, C>(row + 1 * SLAB, vN);
-                    lds_ext<T, C>(row + 2 * SLAB, wN);
-                    lds_ext<T, C>(row + 3 * SLAB, aN);
-                    lds_ext<T, C>(row + 4 * SLAB, bN);
-                    lds_own<T, C>(row + 5 * SLAB, cN);
-                    // mirrored x ghosts of W (tangential difference in H at boundary cells)
-                    if (atW) wN[0] = wN[1];
-                    if (atE) wN[C + 1] = wN[C];
-#pragma unroll
-                    for (int c = 0; c < C; ++c) hN[c] = bN[c + 1] * (wN[c + 2] - wN[c]);
-
-                    const int jc = j0 - 2 + n;  // centre row being computed (valid output if n >= 2)
-                    if (n >= 1) {
-                        // cross term G with mirrored y ghosts (warp-uniform tests)
-                        T G[E];
-                        if (jc == 0) {
-#pragma unroll
-                            for (int e = 0; e < E; ++e) G[e] = bC[e] * (wN[e] - wC[e]);
-                        } else if (jc == ny - 1) {
-#pragma unroll
-                            for (int e = 0; e < E; ++e) G[e] = bC[e] * (wC[e] - wP[e]);
-                        } else {
-#pragma unroll
-                            for (int e = 0; e < E; ++e) G[e] = bC[e] * (wN[e] - wP[e]);
-                        }
-                        // x faces f = 0..C (face f lies between extended cells f and f+1)
-                        T pV[C + 1], pW[C + 1];
-#pragma unroll
-                        for (int f = 0; f <= C; ++f) {
-                            pV[f] = flux_V(uC[f], uC[f + 1], vC[f], vC[f + 1]);
-                            pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1]);
-                        }
-                        if (atW) { pV[0] = (T)0; pW[0] = (T)0; }
-                        if (atE) { pV[C] = (T)0; pW[C] = (T)0; }
-                        // north faces of the own cells; zero on the domain boundary
-                        T nV[C], nW[C];
-                        if (jc >= 0 && jc < ny - 1) {
-#pragma unroll
-                            for (int c = 0; c < C; ++c) {
-                                nV[c] = flux_V(uC[c + 1], uN[c + 1], vC[c + 1], vN[c + 1]);
-                                nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c]);
-                            }
-                        } else {
-#pragma unroll
-                            for (int c = 0; c < C; ++c) nV[c] = nW[c] = (T)0;
-                        }
-                        if (n >= 2) {
-                            T oU[C], oV[C], oW[C];
-#pragma unroll
-                            for (int c = 0; c < C; ++c) {
-                                const T divV = (pV[c + 1] - pV[c]) + (nV[c] - sV[c]);
-                                const T divW = (pW[c + 1] - pW[c]) + (nW[c] - sW[c]);
-                                oU[c] = upd_U(k, uC[c + 1], wC[c + 1]);
-                                oV[c] = upd_V(k, vC[c + 1], divV);
-                                oW[c] = upd_W(k, vC[c + 1], wC[c + 1], divW);
-                            }
-                            if (valid) {
-                                const size_t off = (size_t)jc * nx;
-                                stg_own<T, C>(gU + off, oU);
-                                stg_own<T, C>(gV + off, oV);
-                                stg_own<T, C>(gW + off, oW);
-                            }
-                        }
-#pragma unroll
-                        for (int c = 0; c < C; ++c) { sV[c] = nV[c]; sW[c] = nW[c]; }
-                    }
-                    // roll the window
-#pragma unroll
-                    for (int e = 0; e < E; ++e) {
-                        wP[e] = wC[e]; wC[e] = wN[e];
-                        uC[e] = uN[e]; vC[e] = vN[e]; aC[e] = aN[e]; bC[e] = bN[e];
-                    }
-#pragma unroll
-                    for (int c = 0; c < C; ++c) { cC[c] = cN[c]; hC[c] = hN[c]; }
-                }
-            }
-            // the stage has been read into registers by every lane: refill it
+        for (int q = 0; q < it.nstage; ++q, ++gc) {
+            // keep the ring full: everything up to NST-1 stages ahead of the one consumed now
+            if (lane == 0) produce(gc + NST);
             __syncwarp();
-            if (lane == 0 && q + NST < nstage) issue(q + NST, slot);
+            const uint32_t slot = gc % NST;
+            mbar_wait(full0 + 8u * slot, (gc / NST) & 1u);
+            const char* st = ring + (size_t)slot * STAGE;
+            // Straight-line row body, instantiated twice: GHOST = false for stages that lie
+            // strictly inside the domain (the hot path: no boundary code at all), GHOST = true
+            // for the few stages that contain ghost row -1 or ny.
+            auto row_body = [&](auto ghost_c, const int rr) {
+                constexpr bool GHOST = decltype(ghost_c)::value;
+                // (no join points, so the rolling window is renamed, not
+                // moved, across the unrolled rows).  Arrival index n: arriving row jn = j0-1+n,
+                // centre row jc = jn-1.  Rows outside [j0, j1) are computed but never stored; the
+                // ring always holds finite data (real rows or TMA zero fill).
+                const int n = q * RB + rr;
+                const int jn = j0 - 1 + n;
+                const char* own = st + ownOff + rr * kStripBytes;
+                const char* west = st + wOff + rr * wSR;
+                const char* east = st + eOff + rr * eSR;
+                lds_run<T, C>(own + 0 * SLAB, west + 0 * wSF, east + 0 * eSF, uN);
+                lds_run<T, C>(own + 1 * SLAB, west + 1 * wSF, east + 1 * eSF, vN);
+                lds_run<T, C>(own + 2 * SLAB, west + 2 * wSF, east + 2 * eSF, wN);
+                lds_run<T, C>(own + 3 * SLAB, west + 3 * wSF, east + 3 * eSF, aN);
+                lds_run<T, C>(own + 4 * SLAB, west + 4 * wSF, east + 4 * eSF, bN);
+                lds_own<T, C>(own + 5 * SLAB, cN);
+                // mirrored x ghosts of W (tangential difference in H at boundary cells)
+                if (atW) wN[0] = wN[1];
+                if (atE) wN[C + 1] = wN[C];
+#pragma unroll
+                for (int c = 0; c < C; ++c) hN[c] = bN[c + 1] * (wN[c + 2] - wN[c]);
+                // Ghost rows (warp-uniform, rare): mirror U, V, W evenly and H oddly across the
+                // domain's bottom / top face, which makes that face's V and W fluxes exactly 0
+                // and the tangential difference in G the mirrored one (reading A2).
+                if constexpr (GHOST) {
+                    if (jn == 0) {       // window centre is ghost row -1: mirror of row 0
+#pragma unroll
+                        for (int e = 0; e < E; ++e) { uC[e] = uN[e]; vC[e] = vN[e]; wC[e] = wN[e]; }
+#pragma unroll
+                        for (int c = 0; c < C; ++c) hC[c] = -hN[c];
+                    }
+                    if (jn == ny) {      // arriving row is ghost row ny: mirror of row ny-1
+#pragma unroll
+                        for (int e = 0; e < E; ++e) { uN[e] = uC[e]; vN[e] = vC[e]; wN[e] = wC[e]; }
+#pragma unroll
+                        for (int c = 0; c < C; ++c) hN[c] = -hC[c];
+                    }
+                }
+                // cross term G (rows jc-1, jc+1)
+                T G[E];
+#pragma unroll
+                for (int e = 0; e < E; ++e) G[e] = bC[e] * (wN[e] - wP[e]);
+                // x faces f = 0..C (face f lies between extended cells f and f+1)
+                T pV[C + 1], pW[C + 1];
+#pragma unroll
+                for (int f = 0; f <= C; ++f) {
+                    pV[f] = flux_V(uC[f], uC[f + 1], vC[f], vC[f + 1]);
+                    pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1]);
+                }
+                if (atW) { pV[0] = (T)0; pW[0] = (T)0; }
+                if (atE) { pV[C] = (T)0; pW[C] = (T)0; }
+                // north faces of the own cells (exactly zero on the domain boundary by mirroring)
+                T nV[C], nW[C];
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    nV[c] = flux_V(uC[c + 1], uN[c + 1], vC[c + 1], vN[c + 1]);
+                    nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c]);
+                }
+                T oU[C], oV[C], oW[C];
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    const T divV = (pV[c + 1] - pV[c]) + (nV[c] - sV[c]);
+                    const T divW = (pW[c + 1] - pW[c]) + (nW[c] - sW[c]);
+                    oU[c] = upd_U(k, uC[c + 1], wC[c + 1]);
+                    oV[c] = upd_V(k, vC[c + 1], divV);
+                    oW[c] = upd_W(k, vC[c + 1], wC[c + 1], divW);
+                }
+                if (valid && n >= 2 && n < nr) {
+                    const size_t off = (size_t)(jn - 1) * nx;
+                    stg_own<T, C>(gU + off, oU);
+                    stg_own<T, C>(gV + off, oV);
+                    stg_own<T, C>(gW + off, oW);
+                }
+                // roll the window
+#pragma unroll
+                for (int c = 0; c < C; ++c) { sV[c] = nV[c]; sW[c] = nW[c]; cC[c] = cN[c]; hC[c] = hN[c]; }
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    wP[e] = wC[e]; wC[e] = wN[e];
+                    uC[e] = uN[e]; vC[e] = vN[e]; aC[e] = aN[e]; bC[e] = bN[e];
+                }
+            };
+            const int jfirst = j0 - 1 + q * RB;  // first row arriving in this stage
+            if (jfirst > 0 && jfirst + RB - 1 < ny) {
+#pragma unroll
+                for (int rr = 0; rr < RB; ++rr) row_body(std::false_type{}, rr);
+            } else {
+#pragma unroll
+                for (int rr = 0; rr < RB; ++rr) row_body(std::true_type{}, rr);
+            }
+            // every lane of this warp has the stage in registers: release it
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8u * slot);
         }
     }
 }

@@ -47,7 +47,7 @@ def test_library_has_sm100a_code_and_tma():
     out = subprocess.run([cuobjdump, "-lelf", build.build()], capture_output=True, text=True).stdout
     assert "sm_100a" in out
     sass = subprocess.run([cuobjdump, "-sass", "-fun",
-                           "_ZN2gg14gg_step_streamIdLi2ELi3ELi10EEEvNS_10StreamArgsE", build.LIB],
+                           "_ZN2gg14gg_step_streamIdLi2ELi4ELi8EEEvNS_10StreamArgsE", build.LIB],
                           capture_output=True, text=True).stdout
     assert "UTMALDG" in sass
     assert "DFMA" in sass

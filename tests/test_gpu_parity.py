@@ -129,14 +129,27 @@ def test_odd_width_takes_generic_path(nx, ny):
 
 
 def test_every_stream_variant_and_chunking():
-    wl = workloads.random_problem(42, 200, 150, batch=2)
+    wl = workloads.random_problem(42, 328, 150, batch=2)   # 6 strips: ragged tile columns
     ref = oracle_run(wl, 7)
     for v in range(binding.gg_num_stream_variants()):
-        for ipw in (1, 4, 64):
-            got, _ = gpu_run(wl, 7, kernel="stream",
-                             options=[(binding.GG_OPT_STREAM_VARIANT, v),
-                                      (binding.GG_OPT_ITEMS_PER_WARP, ipw)])
-            assert_close(got, ref, "f64", f"variant {v} items/warp {ipw}")
+        for nw in (0, 1, 2, 4, 8):
+            for ipc in (1, 64):
+                got, _ = gpu_run(wl, 7, kernel="stream",
+                                 options=[(binding.GG_OPT_STREAM_VARIANT, v),
+                                          (binding.GG_OPT_STREAM_WARPS, nw),
+                                          (binding.GG_OPT_ITEMS_PER_WARP, ipc)])
+                assert_close(got, ref, "f64", f"variant {v} warps {nw} items/CTA {ipc}")
+
+
+def test_wide_grid_fp32_and_fp64_all_warp_counts():
+    """1100 fp32 / 1030 fp64 cells per row: several full tile columns plus a ragged last one."""
+    for dtype, nx in (("f32", 1100), ("f64", 1030)):
+        wl = workloads.random_problem(77, nx, 45)
+        ref = oracle_run(wl, 5)
+        for nw in (1, 2, 4, 8):
+            got, _ = gpu_run(wl, 5, dtype=dtype, kernel="stream",
+                             options=[(binding.GG_OPT_STREAM_WARPS, nw)])
+            assert_close(got, ref, dtype, f"{dtype} nx={nx} warps {nw}")
 
 
 def test_stream_and_generic_agree_closely():
