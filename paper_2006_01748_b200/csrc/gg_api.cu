@@ -137,7 +137,7 @@ namespace {
 // v = 0 is the build tuned on B200; the others stay selectable through
 // GG_OPT_STREAM_VARIANT for re-tuning.
 struct Variant { int rb, nst; };
-constexpr Variant kVariants[] = {{2, 4}, {4, 2}, {2, 3}, {1, 6}, {1, 8}, {4, 3}};
+constexpr Variant kVariants[] = {{2, 4}, {4, 2}, {2, 3}, {1, 6}, {1, 8}, {4, 3}, {3, 3}, {3, 2}};
 constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
 constexpr int kDefaultVariant = 1;
 
@@ -161,6 +161,8 @@ int with_variant(int v, int nw, F&& f) {
         case 3: return with_nw<T, 1, 6>(nw, f);
         case 4: return with_nw<T, 1, 8>(nw, f);
         case 5: return nw <= 4 ? with_nw<T, 4, 3>(nw, f) : -1;  // 8 warps would not fit in smem
+        case 6: return with_nw<T, 3, 3>(nw, f);
+        case 7: return with_nw<T, 3, 2>(nw, f);
     }
     return -1;
 }
@@ -227,22 +229,24 @@ int build_plan(gg_ctx* c) {
     if (nw == 0) nw = nstrips >= 8 ? 8 : nstrips >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
     if (c->opt_variant == 5 && nw > 4) nw = 4;
     P.rb = var.rb; P.nst = var.nst; P.nw = nw;
+    const int gw_max = 256 / strip_cells;                 // a TMA box is at most 256 elements wide
+    const int box_bytes = (nw < gw_max ? nw : gw_max) * gg::kStripBytes;
     for (int p = 0; p < 2; ++p)
         for (int f = 0; f < 3; ++f) {
-            int rc = make_map(c, &P.state[p][f], c->state[p][f], c->nbatch, gg::kStripBytes, P.rb);
+            int rc = make_map(c, &P.state[p][f], c->state[p][f], c->nbatch, box_bytes, P.rb);
             if (rc) return rc;
             rc = make_map(c, &P.state_halo[p][f], c->state[p][f], c->nbatch, gg::kHaloBytes, P.rb);
             if (rc) return rc;
         }
     for (int f = 0; f < 3; ++f) {
-        int rc = make_map(c, &P.coef[f], c->coef[f], 1, gg::kStripBytes, P.rb);
+        int rc = make_map(c, &P.coef[f], c->coef[f], 1, box_bytes, P.rb);
         if (rc) return rc;
         if (f < 2) {
             rc = make_map(c, &P.coef_halo[f], c->coef[f], 1, gg::kHaloBytes, P.rb);
             if (rc) return rc;
         }
     }
-    P.block = nw * 32;
+    P.block = (nw + 1) * 32;  // nw consumer warps + the TMA producer warp
     P.smem = (size_t)gg::stream_smem_bytes(P.rb, P.nst, nw);
     const void* fn = nullptr;
     int rc = c->dtype == GG_F64 ? with_variant<double>(c->opt_variant, nw, KernelPtr{&fn})

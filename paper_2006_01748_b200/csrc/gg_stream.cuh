@@ -177,15 +177,23 @@ __device__ __forceinline__ StreamItem stream_item(const StreamArgs& A, long long
 // The kernel.  T: arithmetic/storage type; RB: rows per TMA box (= per ring stage); NST: ring
 // stages; NW: warps (= strips) per CTA.  Dynamic shared memory:
 //   [full[NST], empty[NST] mbarriers, 128 B][NST stages]; a stage is
-//   [NW warps][6 arrays][RB rows][512 B] followed by [west, east][5 arrays][128 B halo slab].
+//   [6 arrays][NG boxes][RB rows][GW strips x 512 B] followed by [west, east][5 arrays][128 B
+//   halo slab]  (GW = strips per TMA box, NG = NW / GW).
 // ------------------------------------------------------------------------------------------
 template <typename T, int RB, int NST, int NW>
-__global__ void __launch_bounds__(NW * 32, 1) gg_step_stream(const __grid_constant__ StreamArgs A) {
+__global__ void __launch_bounds__((NW + 1) * 32, 1) gg_step_stream(const __grid_constant__ StreamArgs A) {
     constexpr int C = 16 / (int)sizeof(T);  // cells per lane per row
     constexpr int SW = 32 * C;              // strip width in cells
     constexpr int E = C + 2;                // extended run: west nbr, C own cells, east nbr
-    constexpr int SLAB = RB * kStripBytes;  // one array of one warp in one stage
-    constexpr int MAIN = NW * 6 * SLAB;
+    // A TMA box may be 256 elements wide, so GW adjacent strips (4 in fp64, 2 in fp32) travel in
+    // one box: fewer, larger TMA instructions for the producer warp.
+    constexpr int GW = (256 / SW) < NW ? (256 / SW) : NW;  // strips per box
+    constexpr int NG = NW / GW;                            // boxes (strip groups) per array
+    constexpr int BOXB = GW * kStripBytes;                 // box row bytes = smem row pitch
+    constexpr int SLABG = RB * BOXB;                       // one box
+    constexpr int ARR = NG * SLABG;                        // one array of the whole tile
+    constexpr int MAIN = 6 * ARR;
+    static_assert(NW % GW == 0, "warps per CTA must be a multiple of the strips per box");
     constexpr int STAGE = stream_stage_bytes(RB, NW);
     static_assert(RB * kHaloBytes <= kHaloSlab, "halo slab too small");
     static_assert(2 * NST * 8 <= 128, "too many stages");
@@ -198,71 +206,70 @@ __global__ void __launch_bounds__(NW * 32, 1) gg_step_stream(const __grid_consta
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NST; ++s) {
-            mbar_init(full0 + 8u * s, NW);
-            mbar_init(empty0 + 8u * s, NW);
+            mbar_init(full0 + 8u * s, 1);    // the producer's arrive.expect_tx (+ the bytes)
+            mbar_init(empty0 + 8u * s, NW);  // one arrival per consumer warp
         }
         fence_barrier_init();
         fence_proxy_async();
     }
     __syncthreads();  // once, before the pipeline starts
 
+    // ---------------------------------------------------------------------------------------
+    // Producer warp (warp NW): walks the same item / stage sequence as the consumers, waits for
+    // a ring slot to be released by all NW consumer warps, then issues the stage's TMA boxes
+    // (6 per strip + 5 per tile-edge halo), spread over its lanes.
+    // ---------------------------------------------------------------------------------------
+    if (warp == NW) {
+        constexpr int NBOX = NG * 6 + 10;
+        constexpr uint32_t STAGE_TX = (uint32_t)(MAIN + 10 * RB * kHaloBytes);
+        uint32_t gp = 0;
+        for (long long item = blockIdx.x; item < A.nitems; item += gridDim.x) {
+            const StreamItem it = stream_item<RB, NW * SW>(A, item);
+            for (int q = 0; q < it.nstage; ++q, ++gp) {
+                const uint32_t slot = gp % NST;
+                if (gp >= NST) mbar_wait(empty0 + 8u * slot, ((gp / NST) - 1u) & 1u);
+                const uint32_t bar = full0 + 8u * slot;
+                const uint32_t dst = ring_u32 + slot * STAGE;
+                const int y = it.j0 - 1 + q * RB;
+                if (lane == 0) mbar_expect_tx(bar, STAGE_TX);
+                __syncwarp();
+                for (int bx = lane; bx < NBOX; bx += 32) {
+                    const CUtensorMap* map;
+                    uint32_t d;
+                    int x, z;
+                    if (bx < NG * 6) {
+                        const int f = bx / NG, g = bx - NG * f;
+                        map = f == 0 ? &A.mU : f == 1 ? &A.mV : f == 2 ? &A.mW : f == 3 ? &A.ma : f == 4 ? &A.mb : &A.mc;
+                        d = dst + f * ARR + g * SLABG;
+                        x = it.i0 + g * GW * SW;
+                        z = f < 3 ? it.sim : 0;
+                    } else {
+                        const int hb = bx - NG * 6, side = hb / 5, f = hb - 5 * side;
+                        map = f == 0 ? &A.hU : f == 1 ? &A.hV : f == 2 ? &A.hW : f == 3 ? &A.ha : &A.hb;
+                        d = dst + MAIN + hb * kHaloSlab;
+                        x = side == 0 ? it.i0 - C : it.i0 + NW * SW;
+                        z = f < 3 ? it.sim : 0;
+                    }
+                    tma_load_3d(d, map, bar, x, y, z);
+                }
+            }
+        }
+        return;
+    }
+
     // per-lane byte offsets inside a stage: own run, west and east neighbour elements
-    const int ownOff = warp * 6 * SLAB + 16 * lane;
+    const int grp = warp / GW, wig = warp % GW;  // strip group (box) and strip within it
+    const int ownOff = grp * SLABG + wig * kStripBytes + 16 * lane;
     int wOff, wSF, wSR, eOff, eSF, eSR;  // offset, stride per array, stride per row
-    if (lane > 0) { wOff = ownOff - (int)sizeof(T); wSF = SLAB; wSR = kStripBytes; }
-    else if (warp > 0) { wOff = (warp - 1) * 6 * SLAB + kStripBytes - (int)sizeof(T); wSF = SLAB; wSR = kStripBytes; }
+    if (lane > 0 || wig > 0) { wOff = ownOff - (int)sizeof(T); wSF = ARR; wSR = BOXB; }
+    else if (grp > 0) { wOff = (grp - 1) * SLABG + BOXB - (int)sizeof(T); wSF = ARR; wSR = BOXB; }
     else { wOff = MAIN + kHaloBytes - (int)sizeof(T); wSF = kHaloSlab; wSR = kHaloBytes; }
-    if (lane < 31) { eOff = ownOff + 16; eSF = SLAB; eSR = kStripBytes; }
-    else if (warp < NW - 1) { eOff = (warp + 1) * 6 * SLAB; eSF = SLAB; eSR = kStripBytes; }
+    if (lane < 31 || wig < GW - 1) { eOff = ownOff + 16; eSF = ARR; eSR = BOXB; }
+    else if (grp < NG - 1) { eOff = (grp + 1) * SLABG; eSF = ARR; eSR = BOXB; }
     else { eOff = MAIN + 5 * kHaloSlab; eSF = kHaloSlab; eSR = kHaloBytes; }
 
     const int nx = A.nx, ny = A.ny;
     const size_t plane = (size_t)nx * ny;
-
-    // producer cursor (lane 0 of every warp issues its own strip): next global stage to issue
-    uint32_t gp = 0;
-    long long p_item = blockIdx.x;
-    int p_q = 0;
-    StreamItem pit = stream_item<RB, NW * SW>(A, p_item < A.nitems ? p_item : 0);
-    // issue global stages up to (but excluding) `limit`
-    auto produce = [&](uint32_t limit) {
-        while (gp < limit && p_item < A.nitems) {
-            const uint32_t slot = gp % NST;
-            if (gp >= NST) mbar_wait(empty0 + 8u * slot, ((gp / NST) - 1u) & 1u);
-            const uint32_t bar = full0 + 8u * slot;
-            const uint32_t dst = ring_u32 + slot * STAGE;
-            const uint32_t mine = dst + warp * 6 * SLAB;
-            const int x = pit.i0 + warp * SW, y = pit.j0 - 1 + p_q * RB, z = pit.sim;
-            uint32_t bytes = 6u * SLAB;
-            if (warp == 0) bytes += 5u * RB * kHaloBytes;
-            if (warp == NW - 1) bytes += 5u * RB * kHaloBytes;
-            mbar_expect_tx(bar, bytes);
-            tma_load_3d(mine + 0 * SLAB, &A.mU, bar, x, y, z);
-            tma_load_3d(mine + 1 * SLAB, &A.mV, bar, x, y, z);
-            tma_load_3d(mine + 2 * SLAB, &A.mW, bar, x, y, z);
-            tma_load_3d(mine + 3 * SLAB, &A.ma, bar, x, y, 0);
-            tma_load_3d(mine + 4 * SLAB, &A.mb, bar, x, y, 0);
-            tma_load_3d(mine + 5 * SLAB, &A.mc, bar, x, y, 0);
-            if (warp == 0 || warp == NW - 1) {
-                for (int side = 0; side < 2; ++side) {
-                    if ((side == 0 && warp != 0) || (side == 1 && warp != NW - 1)) continue;
-                    const uint32_t h = dst + MAIN + side * 5 * kHaloSlab;
-                    const int hx = side == 0 ? pit.i0 - C : pit.i0 + NW * SW;
-                    tma_load_3d(h + 0 * kHaloSlab, &A.hU, bar, hx, y, z);
-                    tma_load_3d(h + 1 * kHaloSlab, &A.hV, bar, hx, y, z);
-                    tma_load_3d(h + 2 * kHaloSlab, &A.hW, bar, hx, y, z);
-                    tma_load_3d(h + 3 * kHaloSlab, &A.ha, bar, hx, y, 0);
-                    tma_load_3d(h + 4 * kHaloSlab, &A.hb, bar, hx, y, 0);
-                }
-            }
-            ++gp;
-            if (++p_q == pit.nstage) {
-                p_q = 0;
-                p_item += gridDim.x;
-                if (p_item < A.nitems) pit = stream_item<RB, NW * SW>(A, p_item);
-            }
-        }
-    };
 
     uint32_t gc = 0;  // global stages consumed (identical sequence in every warp of the CTA)
     for (long long item = blockIdx.x; item < A.nitems; item += gridDim.x) {
@@ -285,9 +292,6 @@ __global__ void __launch_bounds__(NW * 32, 1) gg_step_stream(const __grid_consta
         for (int c = 0; c < C; ++c) cC[c] = hC[c] = sV[c] = sW[c] = (T)0;
 
         for (int q = 0; q < it.nstage; ++q, ++gc) {
-            // keep the ring full: everything up to NST-1 stages ahead of the one consumed now
-            if (lane == 0) produce(gc + NST);
-            __syncwarp();
             const uint32_t slot = gc % NST;
             mbar_wait(full0 + 8u * slot, (gc / NST) & 1u);
             const char* st = ring + (size_t)slot * STAGE;
@@ -302,15 +306,15 @@ __global__ void __launch_bounds__(NW * 32, 1) gg_step_stream(const __grid_consta
                 // ring always holds finite data (real rows or TMA zero fill).
                 const int n = q * RB + rr;
                 const int jn = j0 - 1 + n;
-                const char* own = st + ownOff + rr * kStripBytes;
+                const char* own = st + ownOff + rr * BOXB;
                 const char* west = st + wOff + rr * wSR;
                 const char* east = st + eOff + rr * eSR;
-                lds_run<T, C>(own + 0 * SLAB, west + 0 * wSF, east + 0 * eSF, uN);
-                lds_run<T, C>(own + 1 * SLAB, west + 1 * wSF, east + 1 * eSF, vN);
-                lds_run<T, C>(own + 2 * SLAB, west + 2 * wSF, east + 2 * eSF, wN);
-                lds_run<T, C>(own + 3 * SLAB, west + 3 * wSF, east + 3 * eSF, aN);
-                lds_run<T, C>(own + 4 * SLAB, west + 4 * wSF, east + 4 * eSF, bN);
-                lds_own<T, C>(own + 5 * SLAB, cN);
+                lds_run<T, C>(own + 0 * ARR, west + 0 * wSF, east + 0 * eSF, uN);
+                lds_run<T, C>(own + 1 * ARR, west + 1 * wSF, east + 1 * eSF, vN);
+                lds_run<T, C>(own + 2 * ARR, west + 2 * wSF, east + 2 * eSF, wN);
+                lds_run<T, C>(own + 3 * ARR, west + 3 * wSF, east + 3 * eSF, aN);
+                lds_run<T, C>(own + 4 * ARR, west + 4 * wSF, east + 4 * eSF, bN);
+                lds_own<T, C>(own + 5 * ARR, cN);
                 // mirrored x ghosts of W (tangential difference in H at boundary cells)
                 if (atW) wN[0] = wN[1];
                 if (atE) wN[C + 1] = wN[C];
