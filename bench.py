@@ -163,6 +163,27 @@ def run_reference(args, wl):
 
 
 # ---------------------------------------------------------------------------------------------
+# multi-rank aggregation ("replicas only": ranks never exchange field data)
+# ---------------------------------------------------------------------------------------------
+def max_over_ranks(x, world, device):
+    """MAX of a per-rank scalar over all ranks (identity for world == 1)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as td
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    td.all_reduce(t, op=td.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_glups(cells_per_rank, steps, ms_local, world, device):
+    """Whole-job throughput: every rank advanced `cells_per_rank` cells by `steps` steps; the job
+    took the slowest rank's device time.  Returns (GLUPS, ms_max)."""
+    ms = max_over_ranks(ms_local, world, device)
+    return cells_per_rank * world * steps / (ms * 1e-3) / 1e9, ms
+
+
+# ---------------------------------------------------------------------------------------------
 # GPU leg
 # ---------------------------------------------------------------------------------------------
 def run_ours(args, wl, rank, world, device):
@@ -181,13 +202,6 @@ def run_ours(args, wl, rank, world, device):
         if dist:
             td.barrier()
         torch.cuda.synchronize(device)
-
-    def max_over_ranks(x):
-        if not dist:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=device)
-        td.all_reduce(t, op=td.ReduceOp.MAX)
-        return float(t.item())
 
     sim = binding.Simulation(wl.nx, wl.ny, wl.h, wl.r, wl.d, wl.alpha, wl.c_r, dtype=dtype,
                              batch=wl.batch, device=str(device))
@@ -215,8 +229,7 @@ def run_ours(args, wl, rank, world, device):
             reps.append(sim.last_step_ms())   # CUDA events on libgg's stream around the K launches
             barrier()
     launches = (sim.launches - l0) // args.reps
-    ms = max_over_ranks(float(np.median(reps)))
-    value = cells * world * K / (ms * 1e-3) / 1e9
+    value, ms = job_glups(cells, K, float(np.median(reps)), world, device)
 
     # ---- end to end through the C ABI with host buffers --------------------------------------
     barrier()
@@ -226,7 +239,7 @@ def run_ours(args, wl, rank, world, device):
     sim.step(K, wl.dt)
     binding.gg_get_state_host(sim.ctx, ptr(out["U"]), ptr(out["V"]), ptr(out["W"]))
     torch.cuda.synchronize(device)
-    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e_s = max_over_ranks(time.perf_counter() - t0, world, device)
     es = 8 if dtype == "f64" else 4
     h2d = (3 * wl.nx * wl.ny + 3 * cells) * es
     d2h = 3 * cells * es
