@@ -257,15 +257,30 @@ int build_plan(gg_ctx* c) {
     GG_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, P.block, P.smem));
     if (per_sm < 1) return fail(c, GG_ERR_CUDA, "stream kernel does not fit on an SM");
     const long long resident = (long long)c->num_sms * per_sm;
-    // Row chunks: about opt_items_per_cta items per resident CTA (static round-robin schedule),
-    // none shorter than 16 rows (each chunk re-reads two halo rows and recomputes one).
+    // Row chunks.  The schedule is static round-robin over `resident` CTAs, so the item count
+    // should fill whole waves: among chunk counts that give between 1 and 4*opt items per CTA pick
+    // the one with the best (wave efficiency) x (useful rows / rows loaded), where every chunk
+    // loads two halo rows and recomputes one.  No chunk is shorter than 16 rows.
     P.ntilecols = (nstrips + nw - 1) / nw;
     const long long per = (long long)P.ntilecols * c->nbatch;
-    long long nchunks = ((long long)c->opt_items_per_warp * resident + per - 1) / per;
     const long long max_chunks = (c->ny + 15) / 16;
-    if (nchunks > max_chunks) nchunks = max_chunks;
-    if (nchunks < 1) nchunks = 1;
-    P.chunk_rows = (int)((c->ny + nchunks - 1) / nchunks);
+    const long long target = (long long)c->opt_items_per_warp * resident;
+    long long best_n = 1;
+    double best_score = -1.0;
+    for (long long n = 1; n <= max_chunks; ++n) {
+        const long long rows = (c->ny + n - 1) / n;
+        const long long nch = (c->ny + rows - 1) / rows;  // chunks actually produced
+        if (nch != n) continue;
+        const long long items = per * nch;
+        if (items > 4 * target && n > 1) break;
+        const long long waves = (items + resident - 1) / resident;
+        // ragged last chunk: the slowest CTA still processes `rows` rows per item
+        const double eff = (double)c->ny * per / ((double)waves * resident * rows);
+        double score = eff * (double)rows / (double)(rows + 2);
+        if (items < target) score *= 0.90 + 0.10 * (double)items / (double)target;  // prefer >= target items
+        if (score > best_score + 1e-9) { best_score = score; best_n = nch; }
+    }
+    P.chunk_rows = (int)((c->ny + best_n - 1) / best_n);
     P.nchunks = (c->ny + P.chunk_rows - 1) / P.chunk_rows;
     P.nitems = (long long)P.ntilecols * P.nchunks * c->nbatch;
     P.grid = (int)(P.nitems < resident ? P.nitems : resident);
