@@ -77,7 +77,8 @@ enum {
     GG_OPT_STREAM_VARIANT = 3,  /* tuning: which (rows/box, stages, warps/CTA) build of the STREAM
                                    kernel runs; 0 .. gg_num_stream_variants()-1                  */
     GG_OPT_ITEMS_PER_WARP = 4,  /* tuning: target work items (row chunk x tile column) per resident CTA */
-    GG_OPT_STREAM_WARPS = 5     /* tuning: warps (= 512-byte strips) per CTA: 1, 2, 4, 8; 0 = from nx */
+    GG_OPT_STREAM_WARPS = 5,    /* tuning: warps (= 512-byte strips) per CTA: 1, 2, 4, 8; 0 = from nx */
+    GG_OPT_STREAM2_VARIANT = 6  /* tuning: build of the STREAM2 kernel, 0 .. gg_num_stream2_variants()-1 */
 };
 
 /* One simulation.  nx, ny >= 2 cells; h > 0 the mesh size (dx = dy = h);
@@ -128,7 +129,7 @@ int gg_set_option(gg_ctx* ctx, int option, long long value);
 /* Introspection for benchmarks and tests.
  * gg_kernel_used: GG_KERNEL_* the next gg_step will run (resolves AUTO), or -1.
  * gg_launches:    number of step kernels this context has launched so far (graph replays count
- *                 every kernel node).
+ *                 every kernel node; a GG_KERNEL_STREAM2 launch advances two steps).
  * gg_last_step_ms: device time of the most recent gg_step call, measured with CUDA events
  *                 recorded on the bound stream around its launches; synchronises on the end
  *                 event.  *ms < 0 if no step has run. */
@@ -146,6 +147,7 @@ const char* gg_last_error(const gg_ctx* ctx);
 
 /* Number of STREAM kernel builds selectable with GG_OPT_STREAM_VARIANT. */
 int gg_num_stream_variants(void);
+int gg_num_stream2_variants(void);
 
 /* Library version string, e.g. "gg-b200 0.1 sm_100a". */
 const char* gg_version(void);

@@ -22,7 +22,7 @@ GG_F64, GG_F32 = 0, 1
 GG_OK, GG_ERR_ARG, GG_ERR_STATE, GG_ERR_CUDA, GG_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
 GG_KERNEL_AUTO, GG_KERNEL_GENERIC, GG_KERNEL_STREAM, GG_KERNEL_STREAM2, GG_KERNEL_RESIDENT = range(5)
 GG_OPT_KERNEL, GG_OPT_GRAPH, GG_OPT_GRAPH_CHUNK, GG_OPT_STREAM_VARIANT, GG_OPT_ITEMS_PER_WARP, \
-    GG_OPT_STREAM_WARPS = range(6)
+    GG_OPT_STREAM_WARPS, GG_OPT_STREAM2_VARIANT = range(7)
 
 KERNEL_NAMES = {GG_KERNEL_AUTO: "auto", GG_KERNEL_GENERIC: "generic", GG_KERNEL_STREAM: "stream",
                 GG_KERNEL_STREAM2: "stream2", GG_KERNEL_RESIDENT: "resident"}
@@ -54,6 +54,7 @@ SIGNATURES = {
     "gg_destroy": (ctypes.c_int, [_vp]),
     "gg_last_error": (ctypes.c_char_p, [_vp]),
     "gg_num_stream_variants": (ctypes.c_int, []),
+    "gg_num_stream2_variants": (ctypes.c_int, []),
     "gg_version": (ctypes.c_char_p, []),
 }
 
@@ -175,6 +176,10 @@ def gg_version() -> str:
 
 def gg_num_stream_variants() -> int:
     return int(load().gg_num_stream_variants())
+
+
+def gg_num_stream2_variants() -> int:
+    return int(load().gg_num_stream2_variants())
 
 
 # ---- convenience holder (torch owns device memory and the stream) ------------------------------

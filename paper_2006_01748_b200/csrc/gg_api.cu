@@ -19,6 +19,7 @@
 #include "gg_common.cuh"
 #include "gg_generic.cuh"
 #include "gg_stream.cuh"
+#include "gg_stream2.cuh"
 
 namespace {
 
@@ -60,8 +61,9 @@ struct gg_ctx {
     int opt_items_per_warp = 4;   // work items per resident CTA
     int opt_warps = 0;            // warps (strips) per CTA; 0 = from the grid width
     // stream-kernel plan (tensor maps etc.)
-    gg::StreamPlan plan;
-    bool plan_ready = false;
+    gg::StreamPlan plan, plan2;   // single-step and two-step stream kernels
+    bool plan_ready = false, plan2_ready = false;
+    int opt_variant2 = 0;
     // graphs
     std::map<GraphKey, cudaGraphExec_t> graphs;
     // stats
@@ -167,6 +169,33 @@ int with_variant(int v, int nw, F&& f) {
     return -1;
 }
 
+// Two-step kernel builds: (rows per box, ring0 stages, ring1 stages); NW in {1, 2, 4} warps per
+// step (so 2*NW + 2 warps per CTA).
+struct Variant2 { int rb, nst0, nst1; };
+constexpr Variant2 kVariants2[] = {{4, 2, 2}, {2, 4, 3}, {2, 3, 3}, {3, 2, 2}, {2, 3, 2}};
+constexpr int kNumVariants2 = (int)(sizeof(kVariants2) / sizeof(kVariants2[0]));
+
+template <typename T, int RB, int N0, int N1, typename F>
+int with_nw2(int nw, F&& f) {
+    switch (nw) {
+        case 1: return f.template operator()<T, RB, N0, N1, 1>();
+        case 2: return f.template operator()<T, RB, N0, N1, 2>();
+        case 4: return f.template operator()<T, RB, N0, N1, 4>();
+    }
+    return -1;
+}
+template <typename T, typename F>
+int with_variant2(int v, int nw, F&& f) {
+    switch (v) {
+        case 0: return with_nw2<T, 4, 2, 2>(nw, f);
+        case 1: return with_nw2<T, 2, 4, 3>(nw, f);
+        case 2: return with_nw2<T, 2, 3, 3>(nw, f);
+        case 3: return with_nw2<T, 3, 2, 2>(nw, f);
+        case 4: return with_nw2<T, 2, 3, 2>(nw, f);
+    }
+    return -1;
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -206,29 +235,31 @@ struct KernelPtr {
     template <typename T, int RB, int NST, int NW>
     int operator()() const { *out = (const void*)gg::gg_step_stream<T, RB, NST, NW>; return 0; }
 };
-struct KernelLaunch {
-    const gg::StreamPlan* P;
-    const gg::StreamArgs* a;
-    cudaStream_t stream;
-    template <typename T, int RB, int NST, int NW>
-    int operator()() const {
-        gg::gg_step_stream<T, RB, NST, NW><<<P->grid, P->block, P->smem, stream>>>(*a);
-        return 0;
-    }
+struct Kernel2Ptr {
+    const void** out;
+    template <typename T, int RB, int N0, int N1, int NW>
+    int operator()() const { *out = (const void*)gg::gg_step_stream2<T, RB, N0, N1, NW>; return 0; }
 };
-
-int build_plan(gg_ctx* c) {
-    if (c->plan_ready) return GG_OK;
+// Builds the plan of the single-step (two_step = false) or two-step stream kernel.
+int build_plan(gg_ctx* c, bool two_step) {
+    bool& ready = two_step ? c->plan2_ready : c->plan_ready;
+    if (ready) return GG_OK;
     if (!stream_shape_ok(c))
         return fail(c, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0");
-    gg::StreamPlan& P = c->plan;
-    const Variant var = kVariants[c->opt_variant];
+    gg::StreamPlan& P = two_step ? c->plan2 : c->plan;
     const int strip_cells = gg::kStripBytes / (int)c->esize();
     const int nstrips = (c->nx + strip_cells - 1) / strip_cells;
     int nw = c->opt_warps;
-    if (nw == 0) nw = nstrips >= 8 ? 8 : nstrips >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
-    if (c->opt_variant == 5 && nw > 4) nw = 4;
-    P.rb = var.rb; P.nst = var.nst; P.nw = nw;
+    if (two_step) {
+        const Variant2 var = kVariants2[c->opt_variant2];
+        if (nw == 0 || nw > 4) nw = nstrips >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
+        P.rb = var.rb; P.nst = var.nst0; P.nst1 = var.nst1; P.nw = nw; P.steps = 2;
+    } else {
+        const Variant var = kVariants[c->opt_variant];
+        if (nw == 0) nw = nstrips >= 8 ? 8 : nstrips >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
+        if (c->opt_variant == 5 && nw > 4) nw = 4;
+        P.rb = var.rb; P.nst = var.nst; P.nst1 = 0; P.nw = nw; P.steps = 1;
+    }
     const int gw_max = 256 / strip_cells;                 // a TMA box is at most 256 elements wide
     const int box_bytes = (nw < gw_max ? nw : gw_max) * gg::kStripBytes;
     for (int p = 0; p < 2; ++p)
@@ -241,17 +272,24 @@ int build_plan(gg_ctx* c) {
     for (int f = 0; f < 3; ++f) {
         int rc = make_map(c, &P.coef[f], c->coef[f], 1, box_bytes, P.rb);
         if (rc) return rc;
-        if (f < 2) {
-            rc = make_map(c, &P.coef_halo[f], c->coef[f], 1, gg::kHaloBytes, P.rb);
-            if (rc) return rc;
-        }
+        rc = make_map(c, &P.coef_halo[f], c->coef[f], 1, gg::kHaloBytes, P.rb);
+        if (rc) return rc;
     }
-    P.block = (nw + 1) * 32;  // nw consumer warps + the TMA producer warp
-    P.smem = (size_t)gg::stream_smem_bytes(P.rb, P.nst, nw);
     const void* fn = nullptr;
-    int rc = c->dtype == GG_F64 ? with_variant<double>(c->opt_variant, nw, KernelPtr{&fn})
+    int rc;
+    if (two_step) {
+        P.block = (2 * nw + 2) * 32;  // nw step-1 + nw step-2 warps, halo warp, TMA producer warp
+        P.smem = (size_t)gg::stream2_smem_bytes(P.rb, P.nst, P.nst1, nw);
+        rc = c->dtype == GG_F64 ? with_variant2<double>(c->opt_variant2, nw, Kernel2Ptr{&fn})
+                                : with_variant2<float>(c->opt_variant2, nw, Kernel2Ptr{&fn});
+    } else {
+        P.block = (nw + 1) * 32;  // nw consumer warps + the TMA producer warp
+        P.smem = (size_t)gg::stream_smem_bytes(P.rb, P.nst, nw);
+        rc = c->dtype == GG_F64 ? with_variant<double>(c->opt_variant, nw, KernelPtr{&fn})
                                 : with_variant<float>(c->opt_variant, nw, KernelPtr{&fn});
-    if (rc || !fn) return fail(c, GG_ERR_UNSUPPORTED, "no stream kernel build for variant %d, %d warps", c->opt_variant, nw);
+    }
+    if (rc || !fn) return fail(c, GG_ERR_UNSUPPORTED, "no stream kernel build for this variant with %d warps", nw);
+    P.fn = fn;
     GG_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem));
     int per_sm = 0;
     GG_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, P.block, P.smem));
@@ -276,7 +314,7 @@ int build_plan(gg_ctx* c) {
         const long long waves = (items + resident - 1) / resident;
         // ragged last chunk: the slowest CTA still processes `rows` rows per item
         const double eff = (double)c->ny * per / ((double)waves * resident * rows);
-        double score = eff * (double)rows / (double)(rows + 2);
+        double score = eff * (double)rows / (double)(rows + 2 * P.steps);
         if (items < target) score *= 0.90 + 0.10 * (double)items / (double)target;  // prefer >= target items
         if (score > best_score + 1e-9) { best_score = score; best_n = nch; }
     }
@@ -284,7 +322,7 @@ int build_plan(gg_ctx* c) {
     P.nchunks = (c->ny + P.chunk_rows - 1) / P.chunk_rows;
     P.nitems = (long long)P.ntilecols * P.nchunks * c->nbatch;
     P.grid = (int)(P.nitems < resident ? P.nitems : resident);
-    c->plan_ready = true;
+    ready = true;
     return GG_OK;
 }
 
@@ -304,22 +342,22 @@ int launch_generic(gg_ctx* c, int src, double dt) {
     return GG_OK;
 }
 
-int launch_stream(gg_ctx* c, int src, double dt) {
-    const gg::StreamPlan& P = c->plan;
+// One launch of the single-step or two-step stream kernel from copy `src` into `src^1`.
+int launch_stream(gg_ctx* c, int src, double dt, bool two_step) {
+    const gg::StreamPlan& P = two_step ? c->plan2 : c->plan;
     gg::StreamArgs a;
     a.mU = P.state[src][0]; a.mV = P.state[src][1]; a.mW = P.state[src][2];
     a.ma = P.coef[0]; a.mb = P.coef[1]; a.mc = P.coef[2];
     a.hU = P.state_halo[src][0]; a.hV = P.state_halo[src][1]; a.hW = P.state_halo[src][2];
-    a.ha = P.coef_halo[0]; a.hb = P.coef_halo[1];
+    a.ha = P.coef_halo[0]; a.hb = P.coef_halo[1]; a.hc = P.coef_halo[2];
     a.U1 = c->state[src ^ 1][0]; a.V1 = c->state[src ^ 1][1]; a.W1 = c->state[src ^ 1][2];
     a.sims = c->d_sims;
     a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
     a.ntilecols = P.ntilecols; a.nchunks = P.nchunks; a.chunk_rows = P.chunk_rows;
     a.nitems = P.nitems;
     a.dt = dt; a.inv_h2 = 1.0 / (c->h * c->h);
-    if (c->dtype == GG_F64) with_variant<double>(c->opt_variant, P.nw, KernelLaunch{&P, &a, c->stream});
-    else with_variant<float>(c->opt_variant, P.nw, KernelLaunch{&P, &a, c->stream});
-    GG_CUDA(c, cudaGetLastError());
+    void* params[1] = {&a};
+    GG_CUDA(c, cudaLaunchKernel(P.fn, dim3(P.grid), dim3(P.block), params, P.smem, c->stream));
     return GG_OK;
 }
 
@@ -330,10 +368,29 @@ int launch_step(gg_ctx* c, int kernel, int src, double dt) {
             return c->dtype == GG_F64 ? launch_generic<double>(c, src, dt)
                                       : launch_generic<float>(c, src, dt);
         case GG_KERNEL_STREAM:
-            return launch_stream(c, src, dt);
+            return launch_stream(c, src, dt, false);
         default:
             return fail(c, GG_ERR_UNSUPPORTED, "kernel %d not available", kernel);
     }
+}
+
+// Enqueue `len` time steps starting from ping-pong copy `src`.  GG_KERNEL_STREAM2 advances two
+// steps per launch and finishes an odd count with one single-step launch.  *nlaunch = kernels
+// launched; every launch flips the ping-pong copy.
+int enqueue_steps(gg_ctx* c, int kernel, int src, long long len, double dt, long long* nlaunch) {
+    long long nl = 0;
+    int s = src;
+    while (len > 0) {
+        int rc;
+        if (kernel == GG_KERNEL_STREAM2 && len >= 2) { rc = launch_stream(c, s, dt, true); len -= 2; }
+        else if (kernel == GG_KERNEL_STREAM2) { rc = launch_stream(c, s, dt, false); len -= 1; }
+        else { rc = launch_step(c, kernel, s, dt); len -= 1; }
+        if (rc) return rc;
+        s ^= 1;
+        ++nl;
+    }
+    *nlaunch = nl;
+    return GG_OK;
 }
 
 }  // namespace
@@ -453,6 +510,7 @@ namespace {
 
 // Capture `len` consecutive steps starting from ping-pong copy `src` into an executable graph.
 int capture_graph(gg_ctx* c, int kernel, long long len, double dt, int src, cudaGraphExec_t* out) {
+    long long nl = 0;
     cudaStream_t cap = nullptr;
     GG_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
     cudaStream_t user = c->stream;
@@ -463,8 +521,7 @@ int capture_graph(gg_ctx* c, int kernel, long long len, double dt, int src, cuda
     if (e != cudaSuccess) {
         rc = fail(c, GG_ERR_CUDA, "cudaStreamBeginCapture: %s", cudaGetErrorString(e));
     } else {
-        int s = src;
-        for (long long k = 0; k < len && rc == GG_OK; ++k, s ^= 1) rc = launch_step(c, kernel, s, dt);
+        rc = enqueue_steps(c, kernel, src, len, dt, &nl);
         e = cudaStreamEndCapture(cap, &graph);
         if (rc == GG_OK && e != cudaSuccess)
             rc = fail(c, GG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
@@ -491,10 +548,17 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
     if (n == 0) return GG_OK;
     const int kernel = resolve_kernel(ctx);
-    if (kernel == GG_KERNEL_STREAM) {
-        int rc = build_plan(ctx);
+    if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2) {
+        int rc = build_plan(ctx, false);
         if (rc) return rc;
     }
+    if (kernel == GG_KERNEL_STREAM2) {
+        int rc = build_plan(ctx, true);
+        if (rc) return rc;
+    }
+    auto launches_for = [kernel](long long len) {
+        return kernel == GG_KERNEL_STREAM2 ? len / 2 + (len & 1) : len;
+    };
     GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
     long long left = n;
     if (ctx->opt_graph && n >= 2) {
@@ -511,17 +575,16 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
                 it = ctx->graphs.emplace(key, ex).first;
             }
             GG_CUDA(ctx, cudaGraphLaunch(it->second, ctx->stream));
-            ctx->cur ^= (int)(len & 1);
-            ctx->launches += len;
+            ctx->cur ^= (int)(launches_for(len) & 1);
+            ctx->launches += launches_for(len);
             left -= len;
         }
     } else {
-        for (; left > 0; --left) {
-            int rc = launch_step(ctx, kernel, ctx->cur, dt);
-            if (rc) return rc;
-            ctx->cur ^= 1;
-            ctx->launches += 1;
-        }
+        long long nl = 0;
+        int rc = enqueue_steps(ctx, kernel, ctx->cur, left, dt, &nl);
+        if (rc) return rc;
+        ctx->cur ^= (int)(nl & 1);
+        ctx->launches += nl;
     }
     GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     ctx->timed = true;
@@ -533,7 +596,7 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
     switch (option) {
         case GG_OPT_KERNEL:
             if (value == GG_KERNEL_AUTO || value == GG_KERNEL_GENERIC) break;
-            if (value == GG_KERNEL_STREAM) {
+            if (value == GG_KERNEL_STREAM || value == GG_KERNEL_STREAM2) {
                 if (!stream_shape_ok(ctx))
                     return fail(ctx, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0 (nx = %d)", ctx->nx);
                 break;
@@ -551,6 +614,9 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
         case GG_OPT_ITEMS_PER_WARP:
             if (value < 1 || value > 1024) return fail(ctx, GG_ERR_ARG, "GG_OPT_ITEMS_PER_CTA: 1..1024");
             break;
+        case GG_OPT_STREAM2_VARIANT:
+            if (value < 0 || value >= kNumVariants2) return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM2_VARIANT: 0..%d", kNumVariants2 - 1);
+            break;
         case GG_OPT_STREAM_WARPS:
             if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8)
                 return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_WARPS: 0, 1, 2, 4 or 8");
@@ -564,8 +630,9 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
         case GG_OPT_GRAPH: ctx->opt_graph = (int)value; break;
         case GG_OPT_GRAPH_CHUNK: ctx->opt_chunk = value; break;
         case GG_OPT_STREAM_VARIANT: ctx->opt_variant = (int)value; ctx->plan_ready = false; break;
-        case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = false; break;
-        case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = false; break;
+        case GG_OPT_STREAM2_VARIANT: ctx->opt_variant2 = (int)value; ctx->plan2_ready = false; break;
+        case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = ctx->plan2_ready = false; break;
+        case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = ctx->plan2_ready = false; break;
     }
     return GG_OK;
 }
@@ -597,6 +664,7 @@ int gg_destroy(gg_ctx* ctx) {
 
 const char* gg_last_error(const gg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 int gg_num_stream_variants(void) { return kNumVariants; }
+int gg_num_stream2_variants(void) { return kNumVariants2; }
 const char* gg_version(void) { return "gg-b200 0.1 sm_100a"; }
 
 }  // extern "C"

@@ -34,6 +34,7 @@
 #include <type_traits>
 
 #include "gg_common.cuh"
+#include "gg_march.cuh"
 
 namespace gg {
 
@@ -44,7 +45,7 @@ constexpr int kHaloSlab = 128;     // shared-memory bytes reserved per halo box 
 struct alignas(64) StreamArgs {
     // rank-3 tensor maps {nx, ny, B}: main boxes {512 B, RB, 1}; halo boxes {16 B, RB, 1}
     CUtensorMap mU, mV, mW, ma, mb, mc;
-    CUtensorMap hU, hV, hW, ha, hb;
+    CUtensorMap hU, hV, hW, ha, hb, hc;
     void* U1;                            // outputs [B][ny][nx]
     void* V1;
     void* W1;
@@ -58,12 +59,14 @@ struct alignas(64) StreamArgs {
 // Host-side plan: tensor maps for both ping-pong copies and the launch geometry.
 struct StreamPlan {
     CUtensorMap state[2][3], state_halo[2][3];
-    CUtensorMap coef[3], coef_halo[2];
+    CUtensorMap coef[3], coef_halo[3];
     int ntilecols = 0, nchunks = 0, chunk_rows = 0;
     long long nitems = 0;
     int grid = 0, block = 0;
     size_t smem = 0;
-    int rb = 0, nst = 0, nw = 0;
+    int rb = 0, nst = 0, nst1 = 0, nw = 0;
+    int steps = 1;  // time steps per launch
+    const void* fn = nullptr;
 };
 
 __host__ __device__ constexpr int stream_stage_bytes(int rb, int nw) {
@@ -117,43 +120,9 @@ __device__ __forceinline__ void fence_proxy_async() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
-// 16-byte vector of T
-template <typename T> struct Vec16;
-template <> struct Vec16<double> { using type = double2; };
-template <> struct Vec16<float> { using type = float4; };
-
-template <typename T, int C>
-__device__ __forceinline__ void lds_own(const char* p, T* x) {
-    typename Vec16<T>::type v = *reinterpret_cast<const typename Vec16<T>::type*>(p);
-    if constexpr (C == 2) { x[0] = v.x; x[1] = v.y; }
-    else { x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w; }
-}
-// own C cells into x[1..C], west neighbour into x[0], east neighbour into x[C+1]
-template <typename T, int C>
-__device__ __forceinline__ void lds_ext(const char* p, T* x) {
-    lds_own<T, C>(p, x + 1);
-    x[0] = *reinterpret_cast<const T*>(p - sizeof(T));
-    x[C + 1] = *reinterpret_cast<const T*>(p + 16);
-}
-template <typename T, int C>
-__device__ __forceinline__ void stg_own(T* g, const T* x) {
-    typename Vec16<T>::type v;
-    if constexpr (C == 2) { v.x = x[0]; v.y = x[1]; }
-    else { v.x = x[0]; v.y = x[1]; v.z = x[2]; v.w = x[3]; }
-    *reinterpret_cast<typename Vec16<T>::type*>(g) = v;
-}
-
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// own C cells from `own`, west / east neighbour elements from wherever they live
-template <typename T, int C>
-__device__ __forceinline__ void lds_run(const char* own, const char* west, const char* east, T* x) {
-    lds_own<T, C>(own, x + 1);
-    x[0] = *reinterpret_cast<const T*>(west);
-    x[C + 1] = *reinterpret_cast<const T*>(east);
-}
-
 // One work item of a CTA: simulation `sim`, tile column starting at cell i0, rows [j0, j1).
 struct StreamItem {
     int sim, i0, j0, j1, nr, nstage;
@@ -184,7 +153,6 @@ template <typename T, int RB, int NST, int NW>
 __global__ void __launch_bounds__((NW + 1) * 32, 1) gg_step_stream(const __grid_constant__ StreamArgs A) {
     constexpr int C = 16 / (int)sizeof(T);  // cells per lane per row
     constexpr int SW = 32 * C;              // strip width in cells
-    constexpr int E = C + 2;                // extended run: west nbr, C own cells, east nbr
     // A TMA box may be 256 elements wide, so GW adjacent strips (4 in fp64, 2 in fp32) travel in
     // one box: fewer, larger TMA instructions for the producer warp.
     constexpr int GW = (256 / SW) < NW ? (256 / SW) : NW;  // strips per box
@@ -259,14 +227,14 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) gg_step_stream(const __grid_
 
     // per-lane byte offsets inside a stage: own run, west and east neighbour elements
     const int grp = warp / GW, wig = warp % GW;  // strip group (box) and strip within it
-    const int ownOff = grp * SLABG + wig * kStripBytes + 16 * lane;
-    int wOff, wSF, wSR, eOff, eSF, eSR;  // offset, stride per array, stride per row
-    if (lane > 0 || wig > 0) { wOff = ownOff - (int)sizeof(T); wSF = ARR; wSR = BOXB; }
-    else if (grp > 0) { wOff = (grp - 1) * SLABG + BOXB - (int)sizeof(T); wSF = ARR; wSR = BOXB; }
-    else { wOff = MAIN + kHaloBytes - (int)sizeof(T); wSF = kHaloSlab; wSR = kHaloBytes; }
-    if (lane < 31 || wig < GW - 1) { eOff = ownOff + 16; eSF = ARR; eSR = BOXB; }
-    else if (grp < NG - 1) { eOff = (grp + 1) * SLABG; eSF = ARR; eSR = BOXB; }
-    else { eOff = MAIN + 5 * kHaloSlab; eSF = kHaloSlab; eSR = kHaloBytes; }
+    LaneMap L;
+    L.oOff = grp * SLABG + wig * kStripBytes + 16 * lane; L.oSF = ARR; L.oSR = BOXB;
+    if (lane > 0 || wig > 0) { L.wOff = L.oOff - (int)sizeof(T); L.wSF = ARR; L.wSR = BOXB; }
+    else if (grp > 0) { L.wOff = (grp - 1) * SLABG + BOXB - (int)sizeof(T); L.wSF = ARR; L.wSR = BOXB; }
+    else { L.wOff = MAIN + kHaloBytes - (int)sizeof(T); L.wSF = kHaloSlab; L.wSR = kHaloBytes; }
+    if (lane < 31 || wig < GW - 1) { L.eOff = L.oOff + 16; L.eSF = ARR; L.eSR = BOXB; }
+    else if (grp < NG - 1) { L.eOff = (grp + 1) * SLABG; L.eSF = ARR; L.eSR = BOXB; }
+    else { L.eOff = MAIN + 5 * kHaloSlab; L.eSF = kHaloSlab; L.eSR = kHaloBytes; }
 
     const int nx = A.nx, ny = A.ny;
     const size_t plane = (size_t)nx * ny;
@@ -283,103 +251,32 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) gg_step_stream(const __grid_
         T* gV = (T*)A.V1 + it.sim * plane + iown;
         T* gW = (T*)A.W1 + it.sim * plane + iown;
 
-        // rolling register window (rows jc-1, jc, jc+1 = P, C, N)
-        T wP[E], wC[E], wN[E], uC[E], uN[E], vC[E], vN[E], aC[E], aN[E], bC[E], bN[E];
-        T cC[C], cN[C], hC[C], hN[C], sV[C], sW[C];
-#pragma unroll
-        for (int e = 0; e < E; ++e) wP[e] = wC[e] = uC[e] = vC[e] = aC[e] = bC[e] = (T)0;
-#pragma unroll
-        for (int c = 0; c < C; ++c) cC[c] = hC[c] = sV[c] = sW[c] = (T)0;
+        MarchWindow<T, C> win;  // rolling register window (rows jc-1, jc, jc+1)
+        win.clear();
 
         for (int q = 0; q < it.nstage; ++q, ++gc) {
             const uint32_t slot = gc % NST;
             mbar_wait(full0 + 8u * slot, (gc / NST) & 1u);
             const char* st = ring + (size_t)slot * STAGE;
-            // Straight-line row body, instantiated twice: GHOST = false for stages that lie
-            // strictly inside the domain (the hot path: no boundary code at all), GHOST = true
-            // for the few stages that contain ghost row -1 or ny.
+            // Row body instantiated twice: GHOST = false for stages strictly inside the domain
+            // (the hot path: no boundary code at all), GHOST = true for the few stages that
+            // contain ghost row -1 or ny.  Arrival index n: arriving row jn = j0-1+n, centre row
+            // jn-1.  Rows outside [j0, j1) are computed but never stored; the ring always holds
+            // finite data (real rows or TMA zero fill).
             auto row_body = [&](auto ghost_c, const int rr) {
                 constexpr bool GHOST = decltype(ghost_c)::value;
-                // (no join points, so the rolling window is renamed, not
-                // moved, across the unrolled rows).  Arrival index n: arriving row jn = j0-1+n,
-                // centre row jc = jn-1.  Rows outside [j0, j1) are computed but never stored; the
-                // ring always holds finite data (real rows or TMA zero fill).
                 const int n = q * RB + rr;
                 const int jn = j0 - 1 + n;
-                const char* own = st + ownOff + rr * BOXB;
-                const char* west = st + wOff + rr * wSR;
-                const char* east = st + eOff + rr * eSR;
-                lds_run<T, C>(own + 0 * ARR, west + 0 * wSF, east + 0 * eSF, uN);
-                lds_run<T, C>(own + 1 * ARR, west + 1 * wSF, east + 1 * eSF, vN);
-                lds_run<T, C>(own + 2 * ARR, west + 2 * wSF, east + 2 * eSF, wN);
-                lds_run<T, C>(own + 3 * ARR, west + 3 * wSF, east + 3 * eSF, aN);
-                lds_run<T, C>(own + 4 * ARR, west + 4 * wSF, east + 4 * eSF, bN);
-                lds_own<T, C>(own + 5 * ARR, cN);
-                // mirrored x ghosts of W (tangential difference in H at boundary cells)
-                if (atW) wN[0] = wN[1];
-                if (atE) wN[C + 1] = wN[C];
-#pragma unroll
-                for (int c = 0; c < C; ++c) hN[c] = bN[c + 1] * (wN[c + 2] - wN[c]);
-                // Ghost rows (warp-uniform, rare): mirror U, V, W evenly and H oddly across the
-                // domain's bottom / top face, which makes that face's V and W fluxes exactly 0
-                // and the tangential difference in G the mirrored one (reading A2).
-                if constexpr (GHOST) {
-                    if (jn == 0) {       // window centre is ghost row -1: mirror of row 0
-#pragma unroll
-                        for (int e = 0; e < E; ++e) { uC[e] = uN[e]; vC[e] = vN[e]; wC[e] = wN[e]; }
-#pragma unroll
-                        for (int c = 0; c < C; ++c) hC[c] = -hN[c];
-                    }
-                    if (jn == ny) {      // arriving row is ghost row ny: mirror of row ny-1
-#pragma unroll
-                        for (int e = 0; e < E; ++e) { uN[e] = uC[e]; vN[e] = vC[e]; wN[e] = wC[e]; }
-#pragma unroll
-                        for (int c = 0; c < C; ++c) hN[c] = -hC[c];
-                    }
-                }
-                // cross term G (rows jc-1, jc+1)
-                T G[E];
-#pragma unroll
-                for (int e = 0; e < E; ++e) G[e] = bC[e] * (wN[e] - wP[e]);
-                // x faces f = 0..C (face f lies between extended cells f and f+1)
-                T pV[C + 1], pW[C + 1];
-#pragma unroll
-                for (int f = 0; f <= C; ++f) {
-                    pV[f] = flux_V(uC[f], uC[f + 1], vC[f], vC[f + 1]);
-                    pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1]);
-                }
-                if (atW) { pV[0] = (T)0; pW[0] = (T)0; }
-                if (atE) { pV[C] = (T)0; pW[C] = (T)0; }
-                // north faces of the own cells (exactly zero on the domain boundary by mirroring)
-                T nV[C], nW[C];
-#pragma unroll
-                for (int c = 0; c < C; ++c) {
-                    nV[c] = flux_V(uC[c + 1], uN[c + 1], vC[c + 1], vN[c + 1]);
-                    nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c]);
-                }
+                win.load(st, L, rr, atW, atE);
                 T oU[C], oV[C], oW[C];
-#pragma unroll
-                for (int c = 0; c < C; ++c) {
-                    const T divV = (pV[c + 1] - pV[c]) + (nV[c] - sV[c]);
-                    const T divW = (pW[c + 1] - pW[c]) + (nW[c] - sW[c]);
-                    oU[c] = upd_U(k, uC[c + 1], wC[c + 1]);
-                    oV[c] = upd_V(k, vC[c + 1], divV);
-                    oW[c] = upd_W(k, vC[c + 1], wC[c + 1], divW);
-                }
+                win.template advance<GHOST>(jn, ny, atW, atE, k, oU, oV, oW);
                 if (valid && n >= 2 && n < nr) {
                     const size_t off = (size_t)(jn - 1) * nx;
-                    stg_own<T, C>(gU + off, oU);
-                    stg_own<T, C>(gV + off, oV);
-                    stg_own<T, C>(gW + off, oW);
+                    st_run<T, C>((char*)(gU + off), oU);
+                    st_run<T, C>((char*)(gV + off), oV);
+                    st_run<T, C>((char*)(gW + off), oW);
                 }
-                // roll the window
-#pragma unroll
-                for (int c = 0; c < C; ++c) { sV[c] = nV[c]; sW[c] = nW[c]; cC[c] = cN[c]; hC[c] = hN[c]; }
-#pragma unroll
-                for (int e = 0; e < E; ++e) {
-                    wP[e] = wC[e]; wC[e] = wN[e];
-                    uC[e] = uN[e]; vC[e] = vN[e]; aC[e] = aN[e]; bC[e] = bN[e];
-                }
+                win.roll();
             };
             const int jfirst = j0 - 1 + q * RB;  // first row arriving in this stage
             if (jfirst > 0 && jfirst + RB - 1 < ny) {

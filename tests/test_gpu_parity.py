@@ -14,7 +14,15 @@ from paper_2006_01748_b200 import binding, workloads
 pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-10, "f32": 2e-4}
-KERNELS = {"generic": binding.GG_KERNEL_GENERIC, "stream": binding.GG_KERNEL_STREAM}
+KERNELS = {"generic": binding.GG_KERNEL_GENERIC, "stream": binding.GG_KERNEL_STREAM,
+           "stream2": binding.GG_KERNEL_STREAM2}
+
+
+def expected_launches(kernel, calls):
+    """Kernel launches for a list of gg_step(n) calls: stream2 advances two steps per launch."""
+    if kernel == "stream2":
+        return sum(n // 2 + n % 2 for n in calls)
+    return sum(calls)
 
 
 def oracle_run(wl, steps):
@@ -35,7 +43,7 @@ def gpu_run(wl, steps, dtype="f64", kernel=None, options=(), split=None):
         used = sim.kernel
         launches = sim.launches
         out = sim.get_state_numpy()
-    assert launches == steps
+    assert launches == expected_launches(used, split or [steps])
     return out, used
 
 
@@ -51,7 +59,7 @@ def assert_close(got, ref, dtype, what=""):
 # BASELINE.json configs (0 and 1 at full size and step count; 2-4 at oracle-sized grids with the
 # same recipe, ragged in both directions so that strips, chunks and TMA boxes have partial tails)
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kernel", ["stream", "generic"])
+@pytest.mark.parametrize("kernel", ["stream", "stream2", "generic"])
 def test_config0_full(kernel):
     wl = workloads.make(0)
     got, used = gpu_run(wl, wl.steps, kernel=kernel)
@@ -86,7 +94,7 @@ def test_config2_reduced_d_sweep(d):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("kernel", ["stream", "generic"])
+@pytest.mark.parametrize("kernel", ["stream", "stream2", "generic"])
 def test_config3_reduced_banded(dtype, kernel):
     wl = workloads.make(3, nx=392, ny=250, steps=300)
     got, _ = gpu_run(wl, wl.steps, dtype=dtype, kernel=kernel)
@@ -113,7 +121,7 @@ def test_random_shapes(nx, ny, dtype):
     ref = oracle_run(wl, 9)
     kernels = ["generic"]
     if (nx * (8 if dtype == "f64" else 4)) % 16 == 0:
-        kernels.append("stream")
+        kernels += ["stream", "stream2"]
     for kernel in kernels:
         got, used = gpu_run(wl, 9, dtype=dtype, kernel=kernel)
         assert used == kernel
@@ -150,6 +158,46 @@ def test_wide_grid_fp32_and_fp64_all_warp_counts():
             got, _ = gpu_run(wl, 5, dtype=dtype, kernel="stream",
                              options=[(binding.GG_OPT_STREAM_WARPS, nw)])
             assert_close(got, ref, dtype, f"{dtype} nx={nx} warps {nw}")
+
+
+def test_every_stream2_variant_warps_and_chunking():
+    wl = workloads.random_problem(43, 328, 150, batch=2)   # 6 strips: ragged tile columns
+    ref = {n: oracle_run(wl, n) for n in (6, 7)}
+    for v in range(binding.gg_num_stream2_variants()):
+        for nw in (0, 1, 2, 4):
+            for ipc, n in ((1, 7), (64, 6)):
+                got, used = gpu_run(wl, n, kernel="stream2",
+                                    options=[(binding.GG_OPT_STREAM2_VARIANT, v),
+                                             (binding.GG_OPT_STREAM_WARPS, nw),
+                                             (binding.GG_OPT_ITEMS_PER_WARP, ipc)])
+                assert used == "stream2"
+                assert_close(got, ref[n], "f64", f"stream2 variant {v} warps {nw} items/CTA {ipc}")
+
+
+def test_stream2_wide_ragged_fp32_fp64():
+    for dtype, nx in (("f32", 1100), ("f64", 1030)):
+        wl = workloads.random_problem(78, nx, 45)
+        ref = oracle_run(wl, 6)
+        for nw in (1, 2, 4):
+            got, _ = gpu_run(wl, 6, dtype=dtype, kernel="stream2",
+                             options=[(binding.GG_OPT_STREAM_WARPS, nw)])
+            assert_close(got, ref, dtype, f"stream2 {dtype} nx={nx} warps {nw}")
+
+
+def test_stream2_equals_two_single_steps():
+    """The two-step kernel applies the single-step march twice: same arithmetic, same order."""
+    wl = workloads.make(2, nx=520, ny=300, steps=40)
+    a, _ = gpu_run(wl, 40, kernel="stream2")
+    b, _ = gpu_run(wl, 40, kernel="stream")
+    for x, y in zip(a, b):
+        assert np.max(np.abs(x - y)) <= 1e-14
+    assert_close(a, oracle_run(wl, 40), "f64", "stream2 cfg2")
+
+
+def test_stream2_config4_batch_and_split_calls():
+    wl = workloads.make(4, nx=264, ny=90, batch=5, steps=60)
+    got, _ = gpu_run(wl, 60, kernel="stream2", split=[1, 2, 3, 0, 7, 47])
+    assert_close(got, oracle_run(wl, 60), "f64", "stream2 cfg4 split")
 
 
 def test_stream_and_generic_agree_closely():
