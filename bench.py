@@ -54,10 +54,11 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(dtype):
-    """Per-launch DRAM bytes of the step kernel from the committed ncu capture, or None."""
+def ncu_traffic(kernel, dtype):
+    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the step kernel at
+    8192^2 from the committed `ncu --set full` capture (profiles/ncu_traffic.json), or None."""
     try:
-        return float(json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))[dtype])
+        return float(json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))[f"{kernel}_{dtype}"])
     except Exception:
         return None
 
@@ -206,7 +207,9 @@ def run_ours(args, wl, rank, world, device):
     sim = binding.Simulation(wl.nx, wl.ny, wl.h, wl.r, wl.d, wl.alpha, wl.c_r, dtype=dtype,
                              batch=wl.batch, device=str(device))
     if args.kernel:
-        sim.set_option(binding.GG_OPT_KERNEL, {"generic": 1, "stream": 2}[args.kernel])
+        sim.set_option(binding.GG_OPT_KERNEL, {"generic": binding.GG_KERNEL_GENERIC,
+                                               "stream": binding.GG_KERNEL_STREAM,
+                                               "stream2": binding.GG_KERNEL_STREAM2}[args.kernel])
     # pinned host copies of the inputs (what a host-side caller holds)
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(wl, k), dtype=npd)).pin_memory()
             for k in ("a", "b", "c", "U", "V", "W")}
@@ -289,7 +292,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--kernel", default=None, choices=[None, "generic", "stream"])
+    ap.add_argument("--kernel", default=None, choices=[None, "generic", "stream", "stream2"])
     ap.add_argument("--reps", type=int, default=3)
     ap.add_argument("--n", type=int, default=8192, help="grid edge (8192 = the headline config)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
@@ -324,8 +327,16 @@ def main():
         peak, peak_src = measured_peak()
         cells = wl.nx * wl.ny
         bpc = BYTES_PER_CELL[args.dtype]
-        achieved = cells * bpc / (res["ms"] * 1e-3) / 1e9
-        traffic = ncu_traffic(args.dtype)
+        # roofline of the dominant (only) kernel: ALGORITHMIC bytes one launch accounts for
+        # (72 B x cells x time steps the launch advances) / its average duration.  The two-step
+        # kernel advances two steps per pass over HBM, so this may exceed the copy peak; `traffic`
+        # is what ncu saw the launch really move.
+        launches = max(res["launches"], 1)
+        steps_per_launch = args.steps / launches
+        bytes_per_launch = cells * bpc * steps_per_launch
+        launch_ms = res["ms"] * args.steps / launches
+        achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
+        traffic = ncu_traffic(res["kernel"], args.dtype) if wl.nx == 8192 else None
         line = {
             "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": res["ms"],
@@ -338,7 +349,9 @@ def main():
                        "reps_ms": res["reps_ms"]},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": cells * bpc,
+                         "algorithmic_bytes_per_launch": bytes_per_launch,
+                         "steps_per_launch": steps_per_launch, "launch_ms": launch_ms,
+                         "dram_gbs_actual": (traffic / (launch_ms * 1e-3) / 1e9) if traffic else None,
                          "frac_of_nominal_8000": achieved / 8000.0},
             "e2e": res["e2e"], "gpu_launches": res["launches"], "clocks": res["clocks"],
         }

@@ -63,7 +63,7 @@ struct gg_ctx {
     // stream-kernel plan (tensor maps etc.)
     gg::StreamPlan plan, plan2;   // single-step and two-step stream kernels
     bool plan_ready = false, plan2_ready = false;
-    int opt_variant2 = 0;
+    int opt_variant2 = -1;        // -1 = tuned default for the dtype
     // graphs
     std::map<GraphKey, cudaGraphExec_t> graphs;
     // stats
@@ -119,7 +119,7 @@ bool stream_shape_ok(const gg_ctx* c) { return ((size_t)c->nx * c->esize()) % 16
 
 int resolve_kernel(const gg_ctx* c) {
     if (c->opt_kernel != GG_KERNEL_AUTO) return c->opt_kernel;
-    return stream_shape_ok(c) ? GG_KERNEL_STREAM : GG_KERNEL_GENERIC;
+    return stream_shape_ok(c) ? GG_KERNEL_STREAM2 : GG_KERNEL_GENERIC;
 }
 
 void drop_graphs(gg_ctx* c) {
@@ -250,9 +250,14 @@ int build_plan(gg_ctx* c, bool two_step) {
     const int strip_cells = gg::kStripBytes / (int)c->esize();
     const int nstrips = (c->nx + strip_cells - 1) / strip_cells;
     int nw = c->opt_warps;
+    // Tuned on B200 at 8192^2: fp64 runs 4 rows per box with 4 strips per
+    // step; fp32 runs 3 rows per box with 2 strips (its row body is twice as long per lane, and
+    // the smaller build keeps the three warp roles inside the instruction cache).
+    const int v2 = c->opt_variant2 >= 0 ? c->opt_variant2 : (c->dtype == GG_F64 ? 0 : 3);
     if (two_step) {
-        const Variant2 var = kVariants2[c->opt_variant2];
-        if (nw == 0 || nw > 4) nw = nstrips >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
+        const Variant2 var = kVariants2[v2];
+        const int nw_max = c->opt_variant2 < 0 && c->dtype == GG_F32 ? 2 : 4;
+        if (nw == 0 || nw > 4) nw = nstrips >= 4 && nw_max >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
         P.rb = var.rb; P.nst = var.nst0; P.nst1 = var.nst1; P.nw = nw; P.steps = 2;
     } else {
         const Variant var = kVariants[c->opt_variant];
@@ -280,8 +285,8 @@ int build_plan(gg_ctx* c, bool two_step) {
     if (two_step) {
         P.block = (2 * nw + 2) * 32;  // nw step-1 + nw step-2 warps, halo warp, TMA producer warp
         P.smem = (size_t)gg::stream2_smem_bytes(P.rb, P.nst, P.nst1, nw);
-        rc = c->dtype == GG_F64 ? with_variant2<double>(c->opt_variant2, nw, Kernel2Ptr{&fn})
-                                : with_variant2<float>(c->opt_variant2, nw, Kernel2Ptr{&fn});
+        rc = c->dtype == GG_F64 ? with_variant2<double>(v2, nw, Kernel2Ptr{&fn})
+                                : with_variant2<float>(v2, nw, Kernel2Ptr{&fn});
     } else {
         P.block = (nw + 1) * 32;  // nw consumer warps + the TMA producer warp
         P.smem = (size_t)gg::stream_smem_bytes(P.rb, P.nst, nw);
@@ -615,7 +620,7 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
             if (value < 1 || value > 1024) return fail(ctx, GG_ERR_ARG, "GG_OPT_ITEMS_PER_CTA: 1..1024");
             break;
         case GG_OPT_STREAM2_VARIANT:
-            if (value < 0 || value >= kNumVariants2) return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM2_VARIANT: 0..%d", kNumVariants2 - 1);
+            if (value < -1 || value >= kNumVariants2) return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM2_VARIANT: -1 (tuned default) or 0..%d", kNumVariants2 - 1);
             break;
         case GG_OPT_STREAM_WARPS:
             if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8)

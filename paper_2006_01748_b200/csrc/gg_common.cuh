@@ -4,6 +4,7 @@
 // Scheme: eq. (3) of arXiv 2006.01748 with the stencils of Table 1
 // and Table 2, evaluated in FLUX FORM:
 //
+//   (the code carries 2 phi and 2 F and halves the step coefficients instead, see flux_V)
 //   V face flux   phiE_ij = (1 - (U_ij + U_i+1,j)/2) (V_i+1,j - V_ij)          [Table 1, E entry x h^2]
 //                 phiN_ij = (1 - (U_ij + U_i,j+1)/2) (V_i,j+1 - V_ij)
 //   W cross terms G_ij = b_ij (W_i,j+1 - W_i,j-1),  H_ij = b_ij (W_i+1,j - W_i-1,j)
@@ -33,9 +34,9 @@ struct StepCoef {
     T dt;     // dt
     T ddt;    // d * dt
     T rdt;    // r * dt
-    T adt;    // alpha * dt / h^2
+    T adt;    // alpha * dt / (2 h^2)   (the face fluxes carry a factor 2, see flux_V)
     T crdt;   // c_r * dt
-    T s;      // dt / h^2
+    T s;      // dt / (2 h^2)
 };
 
 template <typename T>
@@ -44,38 +45,58 @@ __device__ __forceinline__ StepCoef<T> fold_coef(const SimScalars& p, double dt,
     k.dt = (T)dt;
     k.ddt = (T)(p.d * dt);
     k.rdt = (T)(p.r * dt);
-    k.adt = (T)(p.alpha * dt * inv_h2);
+    k.adt = (T)(0.5 * p.alpha * dt * inv_h2);
     k.crdt = (T)(p.c_r * dt);
-    k.s = (T)(dt * inv_h2);
+    k.s = (T)(0.5 * dt * inv_h2);
     return k;
 }
 
-// Pointwise pieces used by every kernel.  fma contraction is left to the compiler (tolerances
-// in DESIGN.md section 6 absorb the evaluation order).
+// Arithmetic with the rounding points written out: _rn intrinsics are never contracted or
+// re-associated by the compiler, so every kernel (generic, single-step, two-step, resident;
+// whatever its instantiation) performs the SAME sequence of roundings per cell.  All kernels of
+// the library are therefore bit-identical to one another, and gg_step(n) does not depend on how
+// the n steps are split into launches or calls (tests/test_gpu_parity.py).
+__device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+
+// Face fluxes carry a common factor 2 (flux_V = 2 phi, flux_W = 2 F) that fold_coef puts into
+// adt and s: one multiplication less per face.
 template <typename T>
 __device__ __forceinline__ T upd_U(const StepCoef<T>& k, T u, T w) {
-    // eq. (3) line 1: U + dt U (1-U) - d dt U W
-    return u + u * (k.dt * ((T)1 - u) - k.ddt * w);
+    // eq. (3) line 1: U + dt U (1-U) - d dt U W  =  U + U (dt (1-U) - d dt W)
+    return fma_(u, fma_(k.dt, sub((T)1, u), -mul(k.ddt, w)), u);
 }
 template <typename T>
-__device__ __forceinline__ T upd_V(const StepCoef<T>& k, T v, T div) {
-    // eq. (3) line 2, div = sum of the four face-flux differences (x h^2)
-    return v + k.rdt * v * ((T)1 - v) + k.adt * div;
+__device__ __forceinline__ T upd_V(const StepCoef<T>& k, T v, T div2) {
+    // eq. (3) line 2; div2 = 2 h^2 D1 (sum of the four doubled face-flux differences)
+    return fma_(k.adt, div2, fma_(mul(k.rdt, v), sub((T)1, v), v));
 }
 template <typename T>
-__device__ __forceinline__ T upd_W(const StepCoef<T>& k, T v, T w, T div) {
-    // eq. (3) line 3
-    return w + k.crdt * (v - w) + k.s * div;
+__device__ __forceinline__ T upd_W(const StepCoef<T>& k, T v, T w, T div2) {
+    // eq. (3) line 3; div2 = 2 h^2 D2
+    return fma_(k.s, div2, fma_(k.crdt, sub(v, w), w));
 }
 template <typename T>
 __device__ __forceinline__ T flux_V(T u0, T u1, T v0, T v1) {
-    // Table 1 face weight x h^2 times the V difference across the face (from cell 0 to cell 1)
-    return ((T)1 - (T)0.5 * (u0 + u1)) * (v1 - v0);
+    // 2 x [Table 1 face weight x h^2] x (V difference across the face, from cell 0 to cell 1)
+    return mul(sub((T)2, add(u0, u1)), sub(v1, v0));
 }
 template <typename T>
 __device__ __forceinline__ T flux_W(T k0, T k1, T w0, T w1, T x0, T x1) {
-    // Table 2: face-mean diffusivity times normal difference + mean of the two cross terms / 2
-    return (T)0.5 * (k0 + k1) * (w1 - w0) + (T)0.25 * (x0 + x1);
+    // 2 x [face-mean diffusivity x normal difference + mean of the two cross terms / 2] (Table 2)
+    return fma_(add(k0, k1), sub(w1, w0), mul((T)0.5, add(x0, x1)));
 }
+// cross term b (W_+ - W_-) of one cell (G: y difference, H: x difference)
+template <typename T>
+__device__ __forceinline__ T cross(T b, T wp, T wm) { return mul(b, sub(wp, wm)); }
+// (east - west) + (north - south) of the doubled face fluxes
+template <typename T>
+__device__ __forceinline__ T div4(T e, T w, T n, T s) { return add(sub(e, w), sub(n, s)); }
 
 }  // namespace gg

@@ -55,15 +55,15 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T pW = flux_V(at(U, iw, j), u, at(V, iw, j), v);
     const T pN = flux_V(u, at(U, i, jn), v, at(V, i, jn));
     const T pS = flux_V(at(U, i, js), u, at(V, i, js), v);
-    const T divV = (pE - pW) + (pN - pS);
+    const T divV = div4(pE, pW, pN, pS);
 
     // ---- W: cross terms at the cell and its four edge neighbours (clamped tangential differences)
     const T b0 = at(A.b, i, j);
-    const T G0 = b0 * (wN - wS), H0 = b0 * (wE - wW);
-    const T GE = at(A.b, ie, j) * (wNE - wSE);
-    const T GW = at(A.b, iw, j) * (wNW - wSW);
-    const T HN = at(A.b, i, jn) * (wNE - wNW);
-    const T HS = at(A.b, i, js) * (wSE - wSW);
+    const T G0 = cross(b0, wN, wS), H0 = cross(b0, wE, wW);
+    const T GE = cross(at(A.b, ie, j), wNE, wSE);
+    const T GW = cross(at(A.b, iw, j), wNW, wSW);
+    const T HN = cross(at(A.b, i, jn), wNE, wNW);
+    const T HS = cross(at(A.b, i, js), wSE, wSW);
     const T a0 = at(A.a, i, j), c0 = at(A.c, i, j);
     T fE = flux_W(a0, at(A.a, ie, j), w, wE, G0, GE);
     T fW = flux_W(at(A.a, iw, j), a0, wW, w, GW, G0);
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     if (!hasW) fW = (T)0;
     if (!hasN) fN = (T)0;
     if (!hasS) fS = (T)0;
-    const T divW = (fE - fW) + (fN - fS);
+    const T divW = div4(fE, fW, fN, fS);
 
     const size_t q = sim * plane + (size_t)j * nx + i;
     A.U1[q] = upd_U(k, u, w);

@@ -88,7 +88,7 @@ struct MarchWindow {
         if (atW) wN[0] = wN[1];
         if (atE) wN[C + 1] = wN[C];
 #pragma unroll
-        for (int c = 0; c < C; ++c) hN[c] = bN[c + 1] * (wN[c + 2] - wN[c]);
+        for (int c = 0; c < C; ++c) hN[c] = cross(bN[c + 1], wN[c + 2], wN[c]);
     }
 
     // Advance the centre row (the row below the arriving row `jn`) by one time step into
@@ -113,7 +113,7 @@ struct MarchWindow {
         }
         T G[E];  // cross term of the x faces (rows jc-1, jc+1)
 #pragma unroll
-        for (int e = 0; e < E; ++e) G[e] = bC[e] * (wN[e] - wP[e]);
+        for (int e = 0; e < E; ++e) G[e] = cross(bC[e], wN[e], wP[e]);
         T pV[C + 1], pW[C + 1];  // x faces f = 0..C (face f lies between extended cells f, f+1)
 #pragma unroll
         for (int f = 0; f <= C; ++f) {
@@ -130,8 +130,8 @@ struct MarchWindow {
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-            const T divV = (pV[c + 1] - pV[c]) + (nV[c] - sV[c]);
-            const T divW = (pW[c + 1] - pW[c]) + (nW[c] - sW[c]);
+            const T divV = div4(pV[c + 1], pV[c], nV[c], sV[c]);
+            const T divW = div4(pW[c + 1], pW[c], nW[c], sW[c]);
             oU[c] = upd_U(k, uC[c + 1], wC[c + 1]);
             oV[c] = upd_V(k, vC[c + 1], divV);
             oW[c] = upd_W(k, vC[c + 1], wC[c + 1], divW);
