@@ -51,10 +51,14 @@ struct Padded {
     // i in [-1, nx], j in [-1, ny]
     double& at(int i, int j) { return v[(size_t)(j + 1) * (nx + 2) + (i + 1)]; }
     double at(int i, int j) const { return v[(size_t)(j + 1) * (nx + 2) + (i + 1)]; }
-    void fill(const double* P, double sign) {
-        for (int j = 0; j < ny; ++j)
-            for (int i = 0; i < nx; ++i) at(i, j) = P[(size_t)j * nx + i];
+    // nthreads only splits the row copies (pure data movement) over OpenMP threads.
+    void fill(const double* P, double sign, int nthreads = 1) {
+        (void)nthreads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads)
+#endif
         for (int j = 0; j < ny; ++j) {
+            for (int i = 0; i < nx; ++i) at(i, j) = P[(size_t)j * nx + i];
             at(-1, j) = sign * at(0, j);
             at(nx, j) = sign * at(nx - 1, j);
         }
@@ -156,9 +160,9 @@ int gg_oracle_step(int nx, int ny, double dx, double dy, double r, double d, dou
     std::vector<double> U1(N), V1(N), W1(N);
     for (long long k = 0; k < n; ++k) {
         // O1: ghost frames of the time-k fields
-        pU.fill(U, +1.0);
-        pV.fill(V, +1.0);
-        pW.fill(W, +1.0);
+        pU.fill(U, +1.0, nthreads);
+        pV.fill(V, +1.0, nthreads);
+        pW.fill(W, +1.0, nthreads);
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static) num_threads(nthreads)
 #endif
@@ -175,9 +179,15 @@ int gg_oracle_step(int nx, int ny, double dx, double dy, double r, double d, dou
             }
         }
         // O7: swap; no clamping or positivity fix anywhere
-        std::memcpy(U, U1.data(), N * sizeof(double));
-        std::memcpy(V, V1.data(), N * sizeof(double));
-        std::memcpy(W, W1.data(), N * sizeof(double));
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads)
+#endif
+        for (int j = 0; j < ny; ++j) {
+            const size_t q = (size_t)j * nx, bytes = (size_t)nx * sizeof(double);
+            std::memcpy(U + q, U1.data() + q, bytes);
+            std::memcpy(V + q, V1.data() + q, bytes);
+            std::memcpy(W + q, W1.data() + q, bytes);
+        }
     }
     return 0;
 }
