@@ -93,6 +93,13 @@ int gg_create(gg_ctx** out, int nx, int ny, double h, double r, double d, double
 int gg_create_batch(gg_ctx** out, int nbatch, int nx, int ny, double h, const double* r,
                     const double* d, const double* alpha, const double* c, int dtype);
 
+/* The general mesh of the paper: distinct mesh sizes dx, dy > 0 ("x_i = i dx, y_j = j dy",
+ * PAPER.md:58; Tables 1-2 carry 1/dx^2, 1/dy^2 and 1/(4 dx dy) separately), any
+ * nbatch >= 1.  gg_create / gg_create_batch are this call with dx = dy = h.  The cells tile
+ * [0, nx*dx] x [0, ny*dy].  r, d, alpha, c: HOST arrays [nbatch], copied. */
+int gg_create_xy(gg_ctx** out, int nbatch, int nx, int ny, double dx, double dy, const double* r,
+                 const double* d, const double* alpha, const double* c, int dtype);
+
 /* Bytes of device memory the context needs: two copies of the state (ping-pong), one of the
  * tensor, the per-simulation scalars, plus alignment padding.  0 if ctx is NULL. */
 size_t gg_workspace_bytes(const gg_ctx* ctx);

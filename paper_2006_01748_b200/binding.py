@@ -38,6 +38,9 @@ SIGNATURES = {
     "gg_create_batch": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int,
                                        ctypes.c_int, ctypes.c_double, _dp, _dp, _dp, _dp,
                                        ctypes.c_int]),
+    "gg_create_xy": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                    ctypes.c_double, ctypes.c_double, _dp, _dp, _dp, _dp,
+                                    ctypes.c_int]),
     "gg_workspace_bytes": (ctypes.c_size_t, [_vp]),
     "gg_bind": (ctypes.c_int, [_vp, _vp, ctypes.c_size_t, _vp]),
     "gg_set_tensor": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
@@ -105,6 +108,14 @@ def gg_create_batch(nbatch, nx, ny, h, r, d, alpha, c, dtype=GG_F64):
     keep = [_darr(v, nbatch) for v in (r, d, alpha, c)]
     _check(None, load().gg_create_batch(ctypes.byref(ctx), nbatch, nx, ny, h,
                                         *[k[1] for k in keep], dtype))
+    return ctx
+
+
+def gg_create_xy(nbatch, nx, ny, dx, dy, r, d, alpha, c, dtype=GG_F64):
+    ctx = _vp()
+    keep = [_darr(v, nbatch) for v in (r, d, alpha, c)]
+    _check(None, load().gg_create_xy(ctypes.byref(ctx), nbatch, nx, ny, dx, dy,
+                                     *[k[1] for k in keep], dtype))
     return ctx
 
 
@@ -187,10 +198,11 @@ class Simulation:
     """One context + its torch workspace.  Marshalling only; all arithmetic is in libgg.so.
 
     r, d, alpha, c are scalars or length-`batch` sequences.  `dtype` is "f64" or "f32".
+    `h` is the mesh size dx; pass `dy=` for a non-square mesh.
     """
 
     def __init__(self, nx, ny, h, r, d, alpha, c, dtype="f64", batch=1, device="cuda:0",
-                 stream=None):
+                 stream=None, dy=None):
         import torch
 
         if not torch.cuda.is_available():
@@ -202,7 +214,9 @@ class Simulation:
         self.tdtype = torch.float64 if self.dtype == GG_F64 else torch.float32
         self.npdtype = np.float64 if self.dtype == GG_F64 else np.float32
         torch.cuda.set_device(self.device)
-        self.ctx = gg_create_batch(self.batch, self.nx, self.ny, float(h), r, d, alpha, c, self.dtype)
+        # h is dx; dy defaults to it (square mesh)
+        self.ctx = gg_create_xy(self.batch, self.nx, self.ny, float(h),
+                                float(h if dy is None else dy), r, d, alpha, c, self.dtype)
         nbytes = gg_workspace_bytes(self.ctx)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         base = self.workspace.data_ptr()
@@ -302,7 +316,7 @@ class Simulation:
 def from_workload(wl, dtype="f64", **kw) -> Simulation:
     """Build a Simulation from a `workloads.Workload` and load its tensor and initial state."""
     sim = Simulation(wl.nx, wl.ny, wl.h, wl.r, wl.d, wl.alpha, wl.c_r, dtype=dtype, batch=wl.batch,
-                     **kw)
+                     dy=wl.dy, **kw)
     sim.set_tensor(wl.a, wl.b, wl.c)
     sim.set_state(wl.U, wl.V, wl.W)
     return sim

@@ -42,7 +42,7 @@ struct GraphKey {
 
 struct gg_ctx {
     int nx = 0, ny = 0, nbatch = 1, dtype = GG_F64;
-    double h = 0;
+    double dx = 0, dy = 0;
     std::vector<gg::SimScalars> sims;
     // workspace
     char* ws = nullptr;
@@ -339,7 +339,7 @@ int launch_generic(gg_ctx* c, int src, double dt) {
     a.a = (const T*)c->coef[0]; a.b = (const T*)c->coef[1]; a.c = (const T*)c->coef[2];
     a.sims = c->d_sims;
     a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
-    a.dt = dt; a.inv_h2 = 1.0 / (c->h * c->h);
+    a.dt = dt; a.dx = c->dx; a.dy = c->dy;
     dim3 block(64, 4, 1);
     dim3 grid((c->nx + 63) / 64, (c->ny + 3) / 4, c->nbatch);
     gg::gg_step_generic<T><<<grid, block, 0, c->stream>>>(a);
@@ -360,7 +360,7 @@ int launch_stream(gg_ctx* c, int src, double dt, bool two_step) {
     a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
     a.ntilecols = P.ntilecols; a.nchunks = P.nchunks; a.chunk_rows = P.chunk_rows;
     a.nitems = P.nitems;
-    a.dt = dt; a.inv_h2 = 1.0 / (c->h * c->h);
+    a.dt = dt; a.dx = c->dx; a.dy = c->dy;
     void* params[1] = {&a};
     GG_CUDA(c, cudaLaunchKernel(P.fn, dim3(P.grid), dim3(P.block), params, P.smem, c->stream));
     return GG_OK;
@@ -405,13 +405,14 @@ int enqueue_steps(gg_ctx* c, int kernel, int src, long long len, double dt, long
 // ------------------------------------------------------------------------------------------
 extern "C" {
 
-int gg_create_batch(gg_ctx** out, int nbatch, int nx, int ny, double h, const double* r,
-                    const double* d, const double* alpha, const double* c, int dtype) {
+int gg_create_xy(gg_ctx** out, int nbatch, int nx, int ny, double dx, double dy, const double* r,
+                 const double* d, const double* alpha, const double* c, int dtype) {
     if (!out) return fail(nullptr, GG_ERR_ARG, "gg_create: out is NULL");
     *out = nullptr;
     if (nbatch < 1) return fail(nullptr, GG_ERR_ARG, "gg_create: nbatch %d < 1", nbatch);
     if (nx < 2 || ny < 2) return fail(nullptr, GG_ERR_ARG, "gg_create: nx, ny must be >= 2 (got %d x %d)", nx, ny);
-    if (!(h > 0.0) || !std::isfinite(h)) return fail(nullptr, GG_ERR_ARG, "gg_create: h must be finite and > 0");
+    if (!(dx > 0.0) || !std::isfinite(dx) || !(dy > 0.0) || !std::isfinite(dy))
+        return fail(nullptr, GG_ERR_ARG, "gg_create: mesh sizes must be finite and > 0");
     if (!r || !d || !alpha || !c) return fail(nullptr, GG_ERR_ARG, "gg_create: NULL parameter array");
     if (dtype != GG_F64 && dtype != GG_F32) return fail(nullptr, GG_ERR_UNSUPPORTED, "gg_create: unknown dtype %d", dtype);
     if ((double)nx * ny * nbatch > 2.0e10) return fail(nullptr, GG_ERR_ARG, "gg_create: grid too large");
@@ -420,12 +421,17 @@ int gg_create_batch(gg_ctx** out, int nbatch, int nx, int ny, double h, const do
             return fail(nullptr, GG_ERR_ARG, "gg_create: non-finite parameter for simulation %d", s);
     gg_ctx* ctx = new (std::nothrow) gg_ctx;
     if (!ctx) return fail(nullptr, GG_ERR_ARG, "gg_create: out of host memory");
-    ctx->nx = nx; ctx->ny = ny; ctx->nbatch = nbatch; ctx->h = h; ctx->dtype = dtype;
+    ctx->nx = nx; ctx->ny = ny; ctx->nbatch = nbatch; ctx->dx = dx; ctx->dy = dy; ctx->dtype = dtype;
     ctx->sims.resize(nbatch);
     for (int s = 0; s < nbatch; ++s) ctx->sims[s] = gg::SimScalars{r[s], d[s], alpha[s], c[s]};
     ctx->opt_variant = kDefaultVariant;
     *out = ctx;
     return GG_OK;
+}
+
+int gg_create_batch(gg_ctx** out, int nbatch, int nx, int ny, double h, const double* r,
+                    const double* d, const double* alpha, const double* c, int dtype) {
+    return gg_create_xy(out, nbatch, nx, ny, h, h, r, d, alpha, c, dtype);
 }
 
 int gg_create(gg_ctx** out, int nx, int ny, double h, double r, double d, double alpha, double c,

@@ -34,20 +34,28 @@ struct StepCoef {
     T dt;     // dt
     T ddt;    // d * dt
     T rdt;    // r * dt
-    T adt;    // alpha * dt / (2 h^2)   (the face fluxes carry a factor 2, see flux_V)
+    T adx;    // alpha * dt / (2 dx^2)   (the face fluxes carry a factor 2, see flux_V)
+    T ady;    // alpha * dt / (2 dy^2)
     T crdt;   // c_r * dt
-    T s;      // dt / (2 h^2)
+    T sx;     // dt / (2 dx^2)
+    T sy;     // dt / (2 dy^2)
+    T thx;    // dx / (2 dy): weight of the cross terms G in an x-face flux (1/2 on a square mesh)
+    T thy;    // dy / (2 dx): weight of the cross terms H in a y-face flux
 };
 
 template <typename T>
-__device__ __forceinline__ StepCoef<T> fold_coef(const SimScalars& p, double dt, double inv_h2) {
+__device__ __forceinline__ StepCoef<T> fold_coef(const SimScalars& p, double dt, double dx, double dy) {
     StepCoef<T> k;
     k.dt = (T)dt;
     k.ddt = (T)(p.d * dt);
     k.rdt = (T)(p.r * dt);
-    k.adt = (T)(0.5 * p.alpha * dt * inv_h2);
+    k.adx = (T)(0.5 * p.alpha * dt / (dx * dx));
+    k.ady = (T)(0.5 * p.alpha * dt / (dy * dy));
     k.crdt = (T)(p.c_r * dt);
-    k.s = (T)(0.5 * dt * inv_h2);
+    k.sx = (T)(0.5 * dt / (dx * dx));
+    k.sy = (T)(0.5 * dt / (dy * dy));
+    k.thx = (T)(0.5 * dx / dy);
+    k.thy = (T)(0.5 * dy / dx);
     return k;
 }
 
@@ -73,14 +81,14 @@ __device__ __forceinline__ T upd_U(const StepCoef<T>& k, T u, T w) {
     return fma_(u, fma_(k.dt, sub((T)1, u), -mul(k.ddt, w)), u);
 }
 template <typename T>
-__device__ __forceinline__ T upd_V(const StepCoef<T>& k, T v, T div2) {
-    // eq. (3) line 2; div2 = 2 h^2 D1 (sum of the four doubled face-flux differences)
-    return fma_(k.adt, div2, fma_(mul(k.rdt, v), sub((T)1, v), v));
+__device__ __forceinline__ T upd_V(const StepCoef<T>& k, T v, T fe, T fw, T fn, T fs) {
+    // eq. (3) line 2; fe, fw, fn, fs: doubled fluxes through the east, west, north, south faces
+    return fma_(k.adx, sub(fe, fw), fma_(k.ady, sub(fn, fs), fma_(mul(k.rdt, v), sub((T)1, v), v)));
 }
 template <typename T>
-__device__ __forceinline__ T upd_W(const StepCoef<T>& k, T v, T w, T div2) {
-    // eq. (3) line 3; div2 = 2 h^2 D2
-    return fma_(k.s, div2, fma_(k.crdt, sub(v, w), w));
+__device__ __forceinline__ T upd_W(const StepCoef<T>& k, T v, T w, T fe, T fw, T fn, T fs) {
+    // eq. (3) line 3
+    return fma_(k.sx, sub(fe, fw), fma_(k.sy, sub(fn, fs), fma_(k.crdt, sub(v, w), w)));
 }
 template <typename T>
 __device__ __forceinline__ T flux_V(T u0, T u1, T v0, T v1) {
@@ -88,15 +96,14 @@ __device__ __forceinline__ T flux_V(T u0, T u1, T v0, T v1) {
     return mul(sub((T)2, add(u0, u1)), sub(v1, v0));
 }
 template <typename T>
-__device__ __forceinline__ T flux_W(T k0, T k1, T w0, T w1, T x0, T x1) {
-    // 2 x [face-mean diffusivity x normal difference + mean of the two cross terms / 2] (Table 2)
-    return fma_(add(k0, k1), sub(w1, w0), mul((T)0.5, add(x0, x1)));
+__device__ __forceinline__ T flux_W(T k0, T k1, T w0, T w1, T x0, T x1, T th) {
+    // 2 dn x [face-mean diffusivity x normal gradient + mean of the two cross terms] (Table 2):
+    // (k0+k1)(w1-w0) + th (x0+x1), x = b x (tangential difference of W), th = dn/(2 dt_) with dn
+    // the mesh size normal to the face and dt_ the tangential one (1/2 on a square mesh)
+    return fma_(add(k0, k1), sub(w1, w0), mul(th, add(x0, x1)));
 }
 // cross term b (W_+ - W_-) of one cell (G: y difference, H: x difference)
 template <typename T>
 __device__ __forceinline__ T cross(T b, T wp, T wm) { return mul(b, sub(wp, wm)); }
-// (east - west) + (north - south) of the doubled face fluxes
-template <typename T>
-__device__ __forceinline__ T div4(T e, T w, T n, T s) { return add(sub(e, w), sub(n, s)); }
 
 }  // namespace gg

@@ -24,7 +24,7 @@ struct GenericArgs {
     const T* __restrict__ c;
     const SimScalars* __restrict__ sims;  // [B]
     int nx, ny, nbatch;
-    double dt, inv_h2;
+    double dt, dx, dy;
 };
 
 template <typename T>
@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T* U = A.U + sim * plane;
     const T* V = A.V + sim * plane;
     const T* W = A.W + sim * plane;
-    const StepCoef<T> k = fold_coef<T>(A.sims[sim], A.dt, A.inv_h2);
+    const StepCoef<T> k = fold_coef<T>(A.sims[sim], A.dt, A.dx, A.dy);
 
     const bool hasW = i > 0, hasE = i < nx - 1, hasS = j > 0, hasN = j < ny - 1;
     const int iw = hasW ? i - 1 : i, ie = hasE ? i + 1 : i;
@@ -55,7 +55,6 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T pW = flux_V(at(U, iw, j), u, at(V, iw, j), v);
     const T pN = flux_V(u, at(U, i, jn), v, at(V, i, jn));
     const T pS = flux_V(at(U, i, js), u, at(V, i, js), v);
-    const T divV = div4(pE, pW, pN, pS);
 
     // ---- W: cross terms at the cell and its four edge neighbours (clamped tangential differences)
     const T b0 = at(A.b, i, j);
@@ -65,21 +64,20 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T HN = cross(at(A.b, i, jn), wNE, wNW);
     const T HS = cross(at(A.b, i, js), wSE, wSW);
     const T a0 = at(A.a, i, j), c0 = at(A.c, i, j);
-    T fE = flux_W(a0, at(A.a, ie, j), w, wE, G0, GE);
-    T fW = flux_W(at(A.a, iw, j), a0, wW, w, GW, G0);
-    T fN = flux_W(c0, at(A.c, i, jn), w, wN, H0, HN);
-    T fS = flux_W(at(A.c, i, js), c0, wS, w, HS, H0);
+    T fE = flux_W(a0, at(A.a, ie, j), w, wE, G0, GE, k.thx);
+    T fW = flux_W(at(A.a, iw, j), a0, wW, w, GW, G0, k.thx);
+    T fN = flux_W(c0, at(A.c, i, jn), w, wN, H0, HN, k.thy);
+    T fS = flux_W(at(A.c, i, js), c0, wS, w, HS, H0, k.thy);
     // zero total normal flux through boundary faces (the cross part does not vanish by clamping)
     if (!hasE) fE = (T)0;
     if (!hasW) fW = (T)0;
     if (!hasN) fN = (T)0;
     if (!hasS) fS = (T)0;
-    const T divW = div4(fE, fW, fN, fS);
 
     const size_t q = sim * plane + (size_t)j * nx + i;
     A.U1[q] = upd_U(k, u, w);
-    A.V1[q] = upd_V(k, v, divV);
-    A.W1[q] = upd_W(k, v, w, divW);
+    A.V1[q] = upd_V(k, v, pE, pW, pN, pS);
+    A.W1[q] = upd_W(k, v, w, fE, fW, fN, fS);
 }
 
 }  // namespace gg

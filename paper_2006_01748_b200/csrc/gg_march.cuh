@@ -118,7 +118,7 @@ struct MarchWindow {
 #pragma unroll
         for (int f = 0; f <= C; ++f) {
             pV[f] = flux_V(uC[f], uC[f + 1], vC[f], vC[f + 1]);
-            pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1]);
+            pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1], k.thx);
         }
         if (atW) { pV[0] = (T)0; pW[0] = (T)0; }
         if (atE) { pV[C] = (T)0; pW[C] = (T)0; }
@@ -126,15 +126,13 @@ struct MarchWindow {
 #pragma unroll
         for (int c = 0; c < C; ++c) {
             nV[c] = flux_V(uC[c + 1], uN[c + 1], vC[c + 1], vN[c + 1]);
-            nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c]);
+            nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c], k.thy);
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-            const T divV = div4(pV[c + 1], pV[c], nV[c], sV[c]);
-            const T divW = div4(pW[c + 1], pW[c], nW[c], sW[c]);
             oU[c] = upd_U(k, uC[c + 1], wC[c + 1]);
-            oV[c] = upd_V(k, vC[c + 1], divV);
-            oW[c] = upd_W(k, vC[c + 1], wC[c + 1], divW);
+            oV[c] = upd_V(k, vC[c + 1], pV[c + 1], pV[c], nV[c], sV[c]);
+            oW[c] = upd_W(k, vC[c + 1], wC[c + 1], pW[c + 1], pW[c], nW[c], sW[c]);
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) { sV[c] = nV[c]; sW[c] = nW[c]; }  // next row's south faces

@@ -53,6 +53,11 @@ class Workload:
     steps: int
     dtypes: tuple = ("f64",)
     notes: dict = field(default_factory=dict)
+    hy: float | None = None   # dy when the mesh is not square; None: dy = dx = h
+
+    @property
+    def dy(self) -> float:
+        return self.h if self.hy is None else self.hy
 
     @property
     def cells(self) -> int:
@@ -236,7 +241,7 @@ def make(cfg: int, *, nx: int | None = None, ny: int | None = None, steps: int |
 
 
 def random_problem(seed: int, nx: int, ny: int, *, batch: int = 1, hetero: bool = True,
-                   bmax: float = 0.8):
+                   bmax: float = 0.8, dy_ratio: float = 1.0):
     """Generic seeded smooth-ish random problem for parity tests on odd shapes: positive-definite
     tensor with |b| <= bmax*sqrt(a*c), state in [0,1].  Pure input construction."""
     rng = np.random.default_rng([SEED, 99, seed])
@@ -256,7 +261,8 @@ def random_problem(seed: int, nx: int, ny: int, *, batch: int = 1, hetero: bool 
     d_ = rng.uniform(0.5, 12.0, batch)
     al_ = rng.uniform(1e-4, 2e-3, batch)
     cr_ = rng.uniform(0.5, 2.0, batch)
-    dt = dt_rule(h, float(al_.max()), a, b, c)
+    hy = h * dy_ratio                      # dy = dy_ratio * dx
+    dt = dt_rule(min(h, hy), float(al_.max()), a, b, c)
     return Workload(name=f"random {batch}x{nx}x{ny} seed {seed}", cfg=-1, nx=nx, ny=ny, h=h,
                     batch=batch, r=r_, d=d_, alpha=al_, c_r=cr_, a=a, b=b, c=c, U=U, V=V, W=W,
-                    dt=dt, steps=8)
+                    dt=dt, steps=8, hy=None if dy_ratio == 1.0 else hy)

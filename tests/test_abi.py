@@ -70,6 +70,16 @@ def test_create_validates_arguments():
         assert str(e.value)
 
 
+def test_create_xy_validates_mesh_sizes():
+    ok = binding.gg_create_xy(2, 8, 6, 0.5, 0.25, 1.0, [2.0, 10.0], 1e-3, 1.0)
+    assert binding.gg_workspace_bytes(ok) > 0
+    binding.gg_destroy(ok)
+    for dx, dy in ((0.0, 0.5), (0.5, -1.0), (float("nan"), 0.5), (0.5, float("inf"))):
+        with pytest.raises(binding.GGError) as e:
+            binding.gg_create_xy(1, 8, 6, dx, dy, 1.0, 10.0, 1e-3, 1.0)
+        assert e.value.code == binding.GG_ERR_ARG
+
+
 def test_calls_before_bind_are_state_errors():
     ctx = binding.gg_create(8, 8, 0.5, 1.0, 10.0, 1e-3, 1.0)
     try:

@@ -27,7 +27,7 @@ def expected_launches(kernel, calls):
 
 def oracle_run(wl, steps):
     outs = [oracle.step(wl.U[s], wl.V[s], wl.W[s], wl.a, wl.b, wl.c, r=wl.r[s], d=wl.d[s],
-                        alpha=wl.alpha[s], c_r=wl.c_r[s], n=steps, dt=wl.dt, dx=wl.h)
+                        alpha=wl.alpha[s], c_r=wl.c_r[s], n=steps, dt=wl.dt, dx=wl.h, dy=wl.dy)
             for s in range(wl.batch)]
     return tuple(np.stack([o[f] for o in outs]) for f in range(3))
 
@@ -220,6 +220,26 @@ def test_graph_and_plain_launches_give_identical_bits():
     b, _ = gpu_run(wl, 131, options=[(binding.GG_OPT_GRAPH, 0)])
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("ratio", [0.5, 1.75])
+def test_rectangular_mesh_dx_ne_dy(ratio, dtype):
+    """gg_create_xy: dx != dy.  Tables 1-2 carry 1/dx^2, 1/dy^2 and 1/(4 dx dy)
+    separately; every kernel must weight x faces, y faces and the cross terms accordingly."""
+    wl = workloads.random_problem(5, 328, 150, batch=2, dy_ratio=ratio)
+    ref = oracle_run(wl, 30)
+    outs = []
+    for kernel in ("generic", "stream", "stream2"):
+        got, used = gpu_run(wl, 30, dtype=dtype, kernel=kernel)
+        assert used == kernel
+        assert_close(got, ref, dtype, f"dx != dy ({ratio}) {kernel}")
+        outs.append(got)
+    for f in range(3):
+        assert np.array_equal(outs[0][f], outs[1][f]) and np.array_equal(outs[0][f], outs[2][f])
+    # and the mesh ratio matters: the square-mesh result differs
+    sq = workloads.random_problem(5, 328, 150, batch=2)
+    assert np.max(np.abs(oracle_run(sq, 30)[2] - ref[2])) > 1e-6
 
 
 def test_split_calls_equal_one_call():
