@@ -101,7 +101,7 @@ int gg_create_xy(gg_ctx** out, int nbatch, int nx, int ny, double dx, double dy,
                  const double* d, const double* alpha, const double* c, int dtype);
 
 /* Bytes of device memory the context needs: two copies of the state (ping-pong), one of the
- * tensor, the per-simulation scalars, plus alignment padding.  0 if ctx is NULL. */
+ * tensor, the per-simulation scalars, reduction scratch, plus alignment padding.  0 if ctx is NULL. */
 size_t gg_workspace_bytes(const gg_ctx* ctx);
 
 /* Hand over caller-owned DEVICE memory (>= gg_workspace_bytes, 256-byte aligned) and the stream
@@ -128,6 +128,35 @@ int gg_get_state(gg_ctx* ctx, void* U, void* V, void* W);
 int gg_set_tensor_host(gg_ctx* ctx, const void* a, const void* b, const void* c);
 int gg_set_state_host(gg_ctx* ctx, const void* U, const void* V, const void* W);
 int gg_get_state_host(gg_ctx* ctx, void* U, void* V, void* W);
+
+/* Diagnostics of the current state, reduced on the device (no gg_get_state): the quantities the
+ * paper's experiments read off the fields -- tumour and acid mass, the interstitial gap between
+ * the fronts where both cell densities are ~0 -- plus the extrema that expose
+ * the scheme's known over/undershoots for b != 0.  out: HOST array
+ * [nbatch][GG_DIAG_COUNT] of doubles, slot order GG_DIAG_*: plain sums over cells (multiply by
+ * dx*dy for masses), cell counts as doubles.  eps >= 0 is the gap threshold.  Accumulation is in
+ * double in a fixed order (deterministic).  Synchronises the bound stream. */
+enum {
+    GG_DIAG_SUM_U = 0,   /* sum_ij U                                   */
+    GG_DIAG_SUM_V = 1,   /* sum_ij V                                   */
+    GG_DIAG_SUM_W = 2,   /* sum_ij W                                   */
+    GG_DIAG_GAP = 3,     /* #{(i,j): U < eps and V < eps}              */
+    GG_DIAG_TUMOUR = 4,  /* #{(i,j): V >= 1/2}                         */
+    GG_DIAG_MIN_W = 5,   /* min W (negative: undershoot, reading A7)   */
+    GG_DIAG_MAX_U = 6,   /* max U (> 1: overshoot)                     */
+    GG_DIAG_MAX_W = 7,   /* max W                                      */
+    GG_DIAG_COUNT = 8
+};
+int gg_diagnostics(gg_ctx* ctx, double eps, double* out);
+
+/* Step-size bound for the explicit scheme (PAPER.md:62, :79, :128 say the host recomputes dt "to
+ * ensure numerical stability" and print no formula; reading A6 is used):
+ *     *dt = safety * min(dx,dy)^2 / max(max_s alpha_s, lambda_max),
+ * lambda_max = max over cells of the larger eigenvalue of [[a,b],[b,c]] (eq. (2)),
+ * reduced on the device from the tensor given to gg_set_tensor.  safety <= 1/4 keeps the linear
+ * part L2-stable (max |symbol| <= 8 lambda_max / h^2); BASELINE.json's workloads use 0.2.
+ * lambda_max may be NULL.  Synchronises the bound stream. */
+int gg_max_stable_dt(gg_ctx* ctx, double safety, double* dt, double* lambda_max);
 
 /* Tuning / path selection; see GG_OPT_*.  Returns GG_ERR_UNSUPPORTED for an unknown option or a
  * kernel the context's shape cannot run (the selection is never silently downgraded). */

@@ -93,3 +93,39 @@ def step(U, V, W, a, b, c, *, r: float, d: float, alpha: float, c_r: float, n: i
     if rc != 0:
         raise ValueError("gg_oracle_step: bad argument")
     return U, V, W
+
+
+# ---------------------------------------------------------------------------------------------
+# Reductions next to the step.  Plain NumPy, written out.
+# Pins: tests/test_oracle_pins.py (brute-force loops on tiny grids, eigvalsh, closed forms).
+# ---------------------------------------------------------------------------------------------
+DIAG_NAMES = ("sum_U", "sum_V", "sum_W", "gap_cells", "tumour_cells", "min_W", "max_U", "max_W")
+
+
+def diagnostics(U, V, W, eps: float) -> np.ndarray:
+    """Diagnostics of one state [ny][nx], in the order DIAG_NAMES: the sums of the three fields,
+    the number of interstitial-gap cells (U < eps and V < eps: neither cell type present, the gap
+    between the fronts of PAPER.md:100-111), the number of tumour cells (V >= 1/2), min W, max U,
+    max W.  Everything in fp64."""
+    U, V, W = _c(U), _c(V), _c(W)
+    return np.array([
+        np.sum(U), np.sum(V), np.sum(W),
+        float(np.count_nonzero((U < eps) & (V < eps))),
+        float(np.count_nonzero(V >= 0.5)),
+        np.min(W), np.max(U), np.max(W)], dtype=np.float64)
+
+
+def lambda_max(a, b, c) -> float:
+    """max over cells of the larger eigenvalue of the tensor [[a,b],[b,c]] of eq. (2)
+    (PAPER.md:40): (a+c)/2 + sqrt(((a-c)/2)^2 + b^2)."""
+    a, b, c = _c(a), _c(b), _c(c)
+    return float(np.max(0.5 * (a + c) + np.sqrt((0.5 * (a - c)) ** 2 + b ** 2)))
+
+
+def max_stable_dt(a, b, c, alpha, dx: float, dy: float | None = None, safety: float = 0.2) -> float:
+    """DESIGN.md reading A6 (the paper prints no formula):
+    safety * min(dx,dy)^2 / max(max alpha, lambda_max(A))."""
+    if dy is None:
+        dy = dx
+    rate = max(float(np.max(alpha)), lambda_max(a, b, c))
+    return safety * min(dx, dy) ** 2 / rate

@@ -50,6 +50,8 @@ SIGNATURES = {
     "gg_set_tensor_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_set_state_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_get_state_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
+    "gg_diagnostics": (ctypes.c_int, [_vp, ctypes.c_double, _dp]),
+    "gg_max_stable_dt": (ctypes.c_int, [_vp, ctypes.c_double, _dp, _dp]),
     "gg_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_longlong]),
     "gg_kernel_used": (ctypes.c_int, [_vp]),
     "gg_launches": (ctypes.c_longlong, [_vp]),
@@ -153,6 +155,24 @@ def gg_set_state_host(ctx, U_ptr, V_ptr, W_ptr):
 
 def gg_get_state_host(ctx, U_ptr, V_ptr, W_ptr):
     _check(ctx, load().gg_get_state_host(ctx, U_ptr, V_ptr, W_ptr))
+
+
+GG_DIAG_NAMES = ("sum_U", "sum_V", "sum_W", "gap_cells", "tumour_cells", "min_W", "max_U", "max_W")
+GG_DIAG_COUNT = len(GG_DIAG_NAMES)
+
+
+def gg_diagnostics(ctx, eps: float, nbatch: int) -> np.ndarray:
+    """[nbatch][GG_DIAG_COUNT] doubles, slot order GG_DIAG_NAMES."""
+    out = np.empty((nbatch, GG_DIAG_COUNT), dtype=np.float64)
+    _check(ctx, load().gg_diagnostics(ctx, float(eps), out.ctypes.data_as(_dp)))
+    return out
+
+
+def gg_max_stable_dt(ctx, safety: float):
+    """(dt, lambda_max)."""
+    dt, lam = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(ctx, load().gg_max_stable_dt(ctx, float(safety), ctypes.byref(dt), ctypes.byref(lam)))
+    return float(dt.value), float(lam.value)
 
 
 def gg_set_option(ctx, option: int, value: int):
@@ -272,6 +292,12 @@ class Simulation:
         for x in (U, V, W):
             assert x.dtype == self.npdtype and x.flags["C_CONTIGUOUS"]
         gg_get_state_host(self.ctx, U.ctypes.data, V.ctypes.data, W.ctypes.data)
+
+    def diagnostics(self, eps=1e-2):
+        return gg_diagnostics(self.ctx, eps, self.batch)
+
+    def max_stable_dt(self, safety=0.2):
+        return gg_max_stable_dt(self.ctx, safety)
 
     # options / introspection ------------------------------------------------------------------
     def set_option(self, option, value):

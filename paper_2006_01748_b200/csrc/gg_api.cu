@@ -20,6 +20,7 @@
 #include "gg_generic.cuh"
 #include "gg_stream.cuh"
 #include "gg_stream2.cuh"
+#include "gg_diag.cuh"
 
 namespace {
 
@@ -52,6 +53,7 @@ struct gg_ctx {
     void* state[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
     void* coef[3] = {nullptr, nullptr, nullptr};
     gg::SimScalars* d_sims = nullptr;
+    double* d_scratch = nullptr;
     int cur = 0;  // which ping-pong copy holds the current time level
     // options
     int opt_kernel = GG_KERNEL_AUTO;
@@ -98,8 +100,10 @@ int fail(const gg_ctx* c, int code, const char* fmt, ...) {
     } while (0)
 
 struct Layout {
-    size_t state[2][3], coef[3], sims, total;
+    size_t state[2][3], coef[3], sims, scratch, total;
 };
+// scratch for the reductions of gg_diag.cuh: [nbatch][kDiagMaxBlocks][8] partials + [nbatch][8]
+size_t scratch_doubles(const gg_ctx* c);
 
 Layout layout_of(const gg_ctx* c) {
     Layout L;
@@ -111,8 +115,14 @@ Layout layout_of(const gg_ctx* c) {
     for (int f = 0; f < 3; ++f) { L.coef[f] = off; off += cb; }
     L.sims = off;
     off += align_up((size_t)c->nbatch * sizeof(gg::SimScalars));
+    L.scratch = off;
+    off += align_up(scratch_doubles(c) * sizeof(double));
     L.total = off;
     return L;
+}
+
+size_t scratch_doubles(const gg_ctx* c) {
+    return (size_t)c->nbatch * gg::kDiagMaxBlocks * gg::kDiagCount + (size_t)c->nbatch * gg::kDiagCount;
 }
 
 bool stream_shape_ok(const gg_ctx* c) { return ((size_t)c->nx * c->esize()) % 16 == 0; }
@@ -460,6 +470,7 @@ int gg_bind(gg_ctx* ctx, void* ws, size_t bytes, void* stream) {
         for (int f = 0; f < 3; ++f) ctx->state[p][f] = ctx->ws + L.state[p][f];
     for (int f = 0; f < 3; ++f) ctx->coef[f] = ctx->ws + L.coef[f];
     ctx->d_sims = (gg::SimScalars*)(ctx->ws + L.sims);
+    ctx->d_scratch = (double*)(ctx->ws + L.scratch);
     GG_CUDA(ctx, cudaMemcpyAsync(ctx->d_sims, ctx->sims.data(), ctx->sims.size() * sizeof(gg::SimScalars),
                                  cudaMemcpyHostToDevice, ctx->stream));
     GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // sims is pageable host memory
@@ -645,6 +656,67 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
         case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = ctx->plan2_ready = false; break;
         case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = ctx->plan2_ready = false; break;
     }
+    return GG_OK;
+}
+
+int gg_diagnostics(gg_ctx* ctx, double eps, double* out) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound || !ctx->have_state) return fail(ctx, GG_ERR_STATE, "gg_diagnostics: no state set");
+    if (!out) return fail(ctx, GG_ERR_ARG, "gg_diagnostics: out is NULL");
+    if (!(eps >= 0.0) || !std::isfinite(eps)) return fail(ctx, GG_ERR_ARG, "gg_diagnostics: eps must be finite and >= 0");
+    const size_t plane = ctx->plane();
+    // segment per block: a multiple of the block size, at most kDiagMaxBlocks blocks per simulation
+    size_t seg = (plane + gg::kDiagMaxBlocks - 1) / gg::kDiagMaxBlocks;
+    seg = (seg + gg::kDiagThreads - 1) / gg::kDiagThreads * gg::kDiagThreads;
+    const int nblk = (int)((plane + seg - 1) / seg);
+    double* partial = ctx->d_scratch;
+    double* fin = ctx->d_scratch + (size_t)ctx->nbatch * gg::kDiagMaxBlocks * gg::kDiagCount;
+    void* const* st = ctx->state[ctx->cur];
+    dim3 grid(nblk, ctx->nbatch);
+    if (ctx->dtype == GG_F64)
+        gg::gg_diag_partial<double><<<grid, gg::kDiagThreads, 0, ctx->stream>>>(
+            (const double*)st[0], (const double*)st[1], (const double*)st[2], plane, seg, eps, partial);
+    else
+        gg::gg_diag_partial<float><<<grid, gg::kDiagThreads, 0, ctx->stream>>>(
+            (const float*)st[0], (const float*)st[1], (const float*)st[2], plane, seg, eps, partial);
+    GG_CUDA(ctx, cudaGetLastError());
+    gg::gg_diag_final<<<ctx->nbatch, gg::kDiagThreads, 0, ctx->stream>>>(partial, nblk, fin);
+    GG_CUDA(ctx, cudaGetLastError());
+    GG_CUDA(ctx, cudaMemcpyAsync(out, fin, (size_t)ctx->nbatch * gg::kDiagCount * sizeof(double),
+                                 cudaMemcpyDeviceToHost, ctx->stream));
+    GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return GG_OK;
+}
+
+int gg_max_stable_dt(gg_ctx* ctx, double safety, double* dt, double* lambda_max) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound || !ctx->have_tensor) return fail(ctx, GG_ERR_STATE, "gg_max_stable_dt: no tensor set");
+    if (!dt) return fail(ctx, GG_ERR_ARG, "gg_max_stable_dt: dt is NULL");
+    if (!(safety > 0.0) || !std::isfinite(safety)) return fail(ctx, GG_ERR_ARG, "gg_max_stable_dt: safety must be finite and > 0");
+    const size_t plane = ctx->plane();
+    size_t seg = (plane + gg::kDiagMaxBlocks - 1) / gg::kDiagMaxBlocks;
+    seg = (seg + gg::kDiagThreads - 1) / gg::kDiagThreads * gg::kDiagThreads;
+    const int nblk = (int)((plane + seg - 1) / seg);
+    if (ctx->dtype == GG_F64)
+        gg::gg_lambda_max_partial<double><<<nblk, gg::kDiagThreads, 0, ctx->stream>>>(
+            (const double*)ctx->coef[0], (const double*)ctx->coef[1], (const double*)ctx->coef[2], plane, seg, ctx->d_scratch);
+    else
+        gg::gg_lambda_max_partial<float><<<nblk, gg::kDiagThreads, 0, ctx->stream>>>(
+            (const float*)ctx->coef[0], (const float*)ctx->coef[1], (const float*)ctx->coef[2], plane, seg, ctx->d_scratch);
+    GG_CUDA(ctx, cudaGetLastError());
+    double part[gg::kDiagMaxBlocks];
+    GG_CUDA(ctx, cudaMemcpyAsync(part, ctx->d_scratch, nblk * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    double lam = part[0];
+    for (int q = 1; q < nblk; ++q) lam = part[q] > lam ? part[q] : lam;
+    double amax = ctx->sims[0].alpha;
+    for (const auto& sc : ctx->sims) amax = sc.alpha > amax ? sc.alpha : amax;
+    const double rate = lam > amax ? lam : amax;
+    if (!(rate > 0.0) || !std::isfinite(rate))
+        return fail(ctx, GG_ERR_ARG, "gg_max_stable_dt: max(alpha, lambda_max) = %g is not positive and finite", rate);
+    const double hmin = ctx->dx < ctx->dy ? ctx->dx : ctx->dy;
+    *dt = safety * hmin * hmin / rate;
+    if (lambda_max) *lambda_max = lam;
     return GG_OK;
 }
 

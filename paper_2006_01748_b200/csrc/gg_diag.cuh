@@ -1,0 +1,127 @@
+// gg_diag.cuh -- device-side reductions next to the step:
+//
+//  * gg_diag_partial / gg_diag_final: per-simulation diagnostics of the current state without a
+//    full gg_get_state -- the quantities the paper's experiments read off the fields (tumour and
+//    acid mass, the interstitial gap U ~ 0 and V ~ 0 between the fronts): sums of
+//    U, V, W, the gap and tumour cell counts, and the extrema that show the scheme's documented
+//    over/undershoots (reading A7).
+//  * gg_lambda_max_partial: max over cells of the larger eigenvalue of [[a,b],[b,c]] (eq. (2),
+//    PAPER.md:40), the quantity the explicit step bound needs (DESIGN.md
+//    reading A6).
+//
+// Both are one pass over HBM (24 B per cell), two-stage and DETERMINISTIC: every block reduces a
+// fixed contiguous segment in a fixed order (per-thread strided serial sum, then a shared-memory
+// tree), the partials are combined by one block per simulation in a fixed order.  Accumulation is
+// always in double, whatever the storage type.
+#pragma once
+#include "gg_common.cuh"
+
+namespace gg {
+
+constexpr int kDiagCount = 8;      // == GG_DIAG_COUNT in include/gg.h
+constexpr int kDiagThreads = 256;
+constexpr int kDiagMaxBlocks = 296;  // partial blocks per simulation (2 per SM on B200)
+
+// slot order == GG_DIAG_* in include/gg.h
+enum { kSumU = 0, kSumV, kSumW, kGap, kTumour, kMinW, kMaxU, kMaxW };
+
+struct DiagAcc {
+    double v[kDiagCount];
+    __device__ __forceinline__ void init() {
+        v[kSumU] = v[kSumV] = v[kSumW] = v[kGap] = v[kTumour] = 0.0;
+        v[kMinW] = INFINITY;
+        v[kMaxU] = v[kMaxW] = -INFINITY;
+    }
+    __device__ __forceinline__ void cell(double u, double vv, double w, double eps) {
+        v[kSumU] += u; v[kSumV] += vv; v[kSumW] += w;
+        v[kGap] += (u < eps && vv < eps) ? 1.0 : 0.0;
+        v[kTumour] += (vv >= 0.5) ? 1.0 : 0.0;
+        v[kMinW] = fmin(v[kMinW], w);
+        v[kMaxU] = fmax(v[kMaxU], u);
+        v[kMaxW] = fmax(v[kMaxW], w);
+    }
+    __device__ __forceinline__ void merge(const double* o) {
+        v[kSumU] += o[kSumU]; v[kSumV] += o[kSumV]; v[kSumW] += o[kSumW];
+        v[kGap] += o[kGap]; v[kTumour] += o[kTumour];
+        v[kMinW] = fmin(v[kMinW], o[kMinW]);
+        v[kMaxU] = fmax(v[kMaxU], o[kMaxU]);
+        v[kMaxW] = fmax(v[kMaxW], o[kMaxW]);
+    }
+};
+
+// fixed-order block reduction of `acc` (tree over shared memory); result valid in thread 0
+__device__ __forceinline__ void diag_block_reduce(DiagAcc& acc, double (*sh)[kDiagCount]) {
+    const int t = threadIdx.x;
+#pragma unroll
+    for (int q = 0; q < kDiagCount; ++q) sh[t][q] = acc.v[q];
+    __syncthreads();
+    for (int s = kDiagThreads / 2; s > 0; s >>= 1) {
+        if (t < s) {
+            acc.merge(sh[t + s]);
+#pragma unroll
+            for (int q = 0; q < kDiagCount; ++q) sh[t][q] = acc.v[q];
+        }
+        __syncthreads();
+    }
+}
+
+// grid = (nblk, nbatch).  Block b of simulation s reduces cells [b*seg, min((b+1)*seg, plane)).
+template <typename T>
+__global__ void __launch_bounds__(kDiagThreads)
+gg_diag_partial(const T* __restrict__ U, const T* __restrict__ V, const T* __restrict__ W,
+                size_t plane, size_t seg, double eps, double* __restrict__ partial) {
+    __shared__ double sh[kDiagThreads][kDiagCount];
+    const size_t base = (size_t)blockIdx.y * plane;
+    const size_t lo = (size_t)blockIdx.x * seg;
+    const size_t hi = lo + seg < plane ? lo + seg : plane;
+    DiagAcc acc;
+    acc.init();
+    for (size_t q = lo + threadIdx.x; q < hi; q += kDiagThreads)
+        acc.cell((double)U[base + q], (double)V[base + q], (double)W[base + q], eps);
+    diag_block_reduce(acc, sh);
+    if (threadIdx.x == 0) {
+        double* o = partial + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kDiagCount;
+#pragma unroll
+        for (int q = 0; q < kDiagCount; ++q) o[q] = acc.v[q];
+    }
+}
+
+// grid = nbatch.  Combines the nblk partials of one simulation in a fixed order.
+__global__ void __launch_bounds__(kDiagThreads)
+gg_diag_final(const double* __restrict__ partial, int nblk, double* __restrict__ out) {
+    __shared__ double sh[kDiagThreads][kDiagCount];
+    DiagAcc acc;
+    acc.init();
+    for (int b = threadIdx.x; b < nblk; b += kDiagThreads)
+        acc.merge(partial + ((size_t)blockIdx.x * nblk + b) * kDiagCount);
+    diag_block_reduce(acc, sh);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 0; q < kDiagCount; ++q) out[(size_t)blockIdx.x * kDiagCount + q] = acc.v[q];
+    }
+}
+
+// max over cells of lambda_+ = (a+c)/2 + sqrt(((a-c)/2)^2 + b^2).  grid = nblk; partial[nblk].
+template <typename T>
+__global__ void __launch_bounds__(kDiagThreads)
+gg_lambda_max_partial(const T* __restrict__ a, const T* __restrict__ b, const T* __restrict__ c,
+                      size_t plane, size_t seg, double* __restrict__ partial) {
+    __shared__ double sh[kDiagThreads];
+    const size_t lo = (size_t)blockIdx.x * seg;
+    const size_t hi = lo + seg < plane ? lo + seg : plane;
+    double m = -INFINITY;
+    for (size_t q = lo + threadIdx.x; q < hi; q += kDiagThreads) {
+        const double aa = (double)a[q], bb = (double)b[q], cc = (double)c[q];
+        const double hd = 0.5 * (aa - cc);
+        m = fmax(m, 0.5 * (aa + cc) + sqrt(hd * hd + bb * bb));
+    }
+    sh[threadIdx.x] = m;
+    __syncthreads();
+    for (int s = kDiagThreads / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+
+}  // namespace gg

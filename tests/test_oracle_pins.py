@@ -430,3 +430,69 @@ def test_bad_arguments_rejected():
     z = np.zeros((4, 4))
     with pytest.raises(ValueError):
         oracle.step(z, z, z, z, z, z, r=1, d=1, alpha=1, c_r=1, n=-1, dt=0.1, dx=1.0)
+
+
+# ---------------------------------------------------------------------------------------------
+# Reductions next to the step (NEXT-1 diagnostics, NEXT-2 step bound)
+# ---------------------------------------------------------------------------------------------
+def test_lambda_max_against_library_eigensolver_and_closed_forms():
+    rng = np.random.default_rng(5)
+    a = rng.uniform(5e-3, 2e-2, (7, 9))
+    c = rng.uniform(5e-3, 2e-2, (7, 9))
+    b = rng.uniform(-0.9, 0.9, (7, 9)) * np.sqrt(a * c)
+    mats = np.stack([np.stack([a, b], -1), np.stack([b, c], -1)], -2)     # [...,2,2]
+    lib = float(np.max(np.linalg.eigvalsh(mats)[..., 1]))                 # LAPACK, not the formula
+    assert abs(oracle.lambda_max(a, b, c) - lib) <= 1e-15
+    # closed forms: diagonal tensor -> max(a, c); a = c -> a + |b|
+    assert oracle.lambda_max(np.full((3, 3), 2.0), np.zeros((3, 3)), np.full((3, 3), 5.0)) == 5.0
+    assert abs(oracle.lambda_max(np.full((3, 3), 2.0), np.full((3, 3), -0.5), np.full((3, 3), 2.0)) - 2.5) < 1e-15
+    # config 1: lambda_max = 1.6403124237e-2, dt = 2.9767576160e-3
+    wl = workloads.make(1, nx=16, ny=16)
+    assert abs(oracle.lambda_max(wl.a, wl.b, wl.c) - 1.6403124237e-2) < 1e-11
+    assert abs(oracle.max_stable_dt(wl.a, wl.b, wl.c, wl.alpha, wl.h) - 2.9767576160e-3) < 1e-12
+    # alpha dominates when the tensor is small; dx != dy takes the smaller mesh size
+    assert oracle.max_stable_dt(wl.a * 1e-3, wl.b * 1e-3, wl.c * 1e-3, [1e-3], 0.5, 0.25, safety=0.2) \
+        == 0.2 * 0.25 ** 2 / 1e-3
+
+
+def test_diagnostics_brute_force_and_special_cases():
+    rng = np.random.default_rng(6)
+    U = rng.uniform(0, 0.05, (5, 7)); V = rng.uniform(0, 1, (5, 7)); W = rng.uniform(-1e-3, 1, (5, 7))
+    eps = 0.02
+    got = oracle.diagnostics(U, V, W, eps)
+    su = sv = sw = 0.0
+    gap = tum = 0
+    mnw, mxu, mxw = math.inf, -math.inf, -math.inf
+    for j in range(5):
+        for i in range(7):
+            su += U[j, i]; sv += V[j, i]; sw += W[j, i]
+            gap += int(U[j, i] < eps and V[j, i] < eps)
+            tum += int(V[j, i] >= 0.5)
+            mnw = min(mnw, W[j, i]); mxu = max(mxu, U[j, i]); mxw = max(mxw, W[j, i])
+    np.testing.assert_allclose(got[:3], [su, sv, sw], rtol=1e-14)
+    assert (got[3], got[4], got[5], got[6], got[7]) == (gap, tum, mnw, mxu, mxw)
+    # the healthy state (1,0,0): no gap, no tumour; the invaded state (0,1,1): no gap, all tumour;
+    # (0,0,w): every cell is gap
+    n = 12
+    one, zero = np.ones((3, 4)), np.zeros((3, 4))
+    assert list(oracle.diagnostics(one, zero, zero, 1e-2)) == [n, 0, 0, 0, 0, 0, 1, 0]
+    assert list(oracle.diagnostics(zero, one, one, 1e-2)) == [0, n, n, 0, n, 1, 0, 1]
+    assert oracle.diagnostics(zero, zero, one * 0.3, 1e-2)[3] == n
+    # thresholds are strict / inclusive as documented: U == eps is not gap, V == 1/2 is tumour
+    assert oracle.diagnostics(one * 1e-2, zero, zero, 1e-2)[3] == 0
+    assert oracle.diagnostics(zero, one * 0.5, zero, 1e-2)[4] == n
+
+
+def test_gap_opens_for_large_d_only():
+    """d > 1 (homogeneous invasion) leaves an interstitial gap between the
+    fronts, d < 1 (heterogeneous invasion) does not: normal cells coexist behind the front.
+    Noise-free disk data (the configs' V noise seeds tumour growth everywhere)."""
+    wl = workloads.make(0)
+    inside = wl.V[0] > 0.5
+    U0, V0, W0 = np.where(inside, 0.0, 1.0), np.where(inside, 1.0, 0.0), np.zeros(inside.shape)
+    gaps = {}
+    for d in (0.5, 40.0):
+        U, V, W = oracle.step(U0, V0, W0, wl.a, wl.b, wl.c, r=1.0, d=d, alpha=1e-3, c_r=1.0, n=600,
+                              dt=wl.dt, dx=wl.h)
+        gaps[d] = oracle.diagnostics(U, V, W, 0.2)[3]
+    assert gaps[0.5] == 0 and gaps[40.0] > 100
