@@ -68,7 +68,9 @@ enum {
     GG_KERNEL_STREAM = 2,   /* TMA-staged shared-memory row ring, register-rolling y march;     */
                             /* needs nx*sizeof(elem) % 16 == 0                                  */
     GG_KERNEL_STREAM2 = 3,  /* as STREAM with two time steps fused per launch (temporal block)  */
-    GG_KERNEL_RESIDENT = 4  /* whole state resident on-chip across steps (small grids)          */
+    GG_KERNEL_RESIDENT = 4, /* whole state resident on-chip across steps (small grids; reserved)*/
+    GG_KERNEL_PAIR = 5      /* two time steps per launch chained in REGISTERS, x-neighbours by  */
+                            /* warp shuffle (gg_pair.cuh); needs nx*sizeof(elem) % 16 == 0      */
 };
 enum {
     GG_OPT_KERNEL = 0,      /* one of GG_KERNEL_*                                               */
@@ -77,8 +79,9 @@ enum {
     GG_OPT_STREAM_VARIANT = 3,  /* tuning: which (rows/box, stages, warps/CTA) build of the STREAM
                                    kernel runs; 0 .. gg_num_stream_variants()-1                  */
     GG_OPT_ITEMS_PER_WARP = 4,  /* tuning: target work items (row chunk x tile column) per resident CTA */
-    GG_OPT_STREAM_WARPS = 5,    /* tuning: warps (= 512-byte strips) per CTA: 1, 2, 4, 8; 0 = from nx */
-    GG_OPT_STREAM2_VARIANT = 6  /* tuning: build of the STREAM2 kernel, 0 .. gg_num_stream2_variants()-1 */
+    GG_OPT_STREAM_WARPS = 5,    /* tuning: warps (= strips) per CTA: STREAM 1, 2, 4, 8; STREAM2 1, 2, 4; PAIR 1..8; 0 = from nx */
+    GG_OPT_STREAM2_VARIANT = 6, /* tuning: build of the STREAM2 kernel, 0 .. gg_num_stream2_variants()-1; -1 = tuned default */
+    GG_OPT_PAIR_VARIANT = 7     /* tuning: build of the PAIR kernel, 0 .. gg_num_pair_variants()-1; -1 = deepest ring that fits */
 };
 
 /* One simulation.  nx, ny >= 2 cells; h > 0 the mesh size (dx = dy = h);
@@ -184,6 +187,7 @@ const char* gg_last_error(const gg_ctx* ctx);
 /* Number of STREAM kernel builds selectable with GG_OPT_STREAM_VARIANT. */
 int gg_num_stream_variants(void);
 int gg_num_stream2_variants(void);
+int gg_num_pair_variants(void);
 
 /* Library version string, e.g. "gg-b200 0.1 sm_100a". */
 const char* gg_version(void);

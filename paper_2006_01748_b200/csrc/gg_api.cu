@@ -21,6 +21,7 @@
 #include "gg_stream.cuh"
 #include "gg_stream2.cuh"
 #include "gg_diag.cuh"
+#include "gg_pair.cuh"
 
 namespace {
 
@@ -65,6 +66,16 @@ struct gg_ctx {
     // stream-kernel plan (tensor maps etc.)
     gg::StreamPlan plan, plan2;   // single-step and two-step stream kernels
     bool plan_ready = false, plan2_ready = false;
+    // register-chained two-step kernel (gg_pair.cuh)
+    struct PairPlan {
+        CUtensorMap state[2][3], coef[3];
+        int nw = 0, ntilecols = 0, nchunks = 0, chunk_rows = 0, grid = 0, block = 0, rb = 0, nst = 0;
+        long long nitems = 0;
+        size_t smem = 0;
+        const void* fn = nullptr;
+        bool ready = false;
+    } pair;
+    int opt_pair_variant = -1;
     int opt_variant2 = -1;        // -1 = tuned default for the dtype
     // graphs
     std::map<GraphKey, cudaGraphExec_t> graphs;
@@ -260,6 +271,7 @@ int build_plan(gg_ctx* c, bool two_step) {
     const int strip_cells = gg::kStripBytes / (int)c->esize();
     const int nstrips = (c->nx + strip_cells - 1) / strip_cells;
     int nw = c->opt_warps;
+    if (resolve_kernel(c) == GG_KERNEL_PAIR) nw = 0;  // GG_OPT_STREAM_WARPS then addresses the pair kernel
     // Tuned on B200 at 8192^2: fp64 runs 4 rows per box with 4 strips per
     // step; fp32 runs 3 rows per box with 2 strips (its row body is twice as long per lane, and
     // the smaller build keeps the three warp roles inside the instruction cache).
@@ -341,6 +353,8 @@ int build_plan(gg_ctx* c, bool two_step) {
     return GG_OK;
 }
 
+#include "gg_pair_plan.inc"
+
 template <typename T>
 int launch_generic(gg_ctx* c, int src, double dt) {
     gg::GenericArgs<T> a;
@@ -398,7 +412,8 @@ int enqueue_steps(gg_ctx* c, int kernel, int src, long long len, double dt, long
     while (len > 0) {
         int rc;
         if (kernel == GG_KERNEL_STREAM2 && len >= 2) { rc = launch_stream(c, s, dt, true); len -= 2; }
-        else if (kernel == GG_KERNEL_STREAM2) { rc = launch_stream(c, s, dt, false); len -= 1; }
+        else if (kernel == GG_KERNEL_PAIR && len >= 2) { rc = launch_pair(c, s, dt); len -= 2; }
+        else if (kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR) { rc = launch_stream(c, s, dt, false); len -= 1; }
         else { rc = launch_step(c, kernel, s, dt); len -= 1; }
         if (rc) return rc;
         s ^= 1;
@@ -570,8 +585,12 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
     if (n == 0) return GG_OK;
     const int kernel = resolve_kernel(ctx);
-    if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2) {
+    if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR) {
         int rc = build_plan(ctx, false);
+        if (rc) return rc;
+    }
+    if (kernel == GG_KERNEL_PAIR) {
+        int rc = build_plan_pair(ctx);
         if (rc) return rc;
     }
     if (kernel == GG_KERNEL_STREAM2) {
@@ -579,7 +598,7 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
         if (rc) return rc;
     }
     auto launches_for = [kernel](long long len) {
-        return kernel == GG_KERNEL_STREAM2 ? len / 2 + (len & 1) : len;
+        return kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ? len / 2 + (len & 1) : len;
     };
     GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
     long long left = n;
@@ -618,7 +637,7 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
     switch (option) {
         case GG_OPT_KERNEL:
             if (value == GG_KERNEL_AUTO || value == GG_KERNEL_GENERIC) break;
-            if (value == GG_KERNEL_STREAM || value == GG_KERNEL_STREAM2) {
+            if (value == GG_KERNEL_STREAM || value == GG_KERNEL_STREAM2 || value == GG_KERNEL_PAIR) {
                 if (!stream_shape_ok(ctx))
                     return fail(ctx, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0 (nx = %d)", ctx->nx);
                 break;
@@ -640,8 +659,11 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
             if (value < -1 || value >= kNumVariants2) return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM2_VARIANT: -1 (tuned default) or 0..%d", kNumVariants2 - 1);
             break;
         case GG_OPT_STREAM_WARPS:
-            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8)
-                return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_WARPS: 0, 1, 2, 4 or 8");
+            if (value < 0 || value > 8)
+                return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_WARPS: 0..8");
+            break;
+        case GG_OPT_PAIR_VARIANT:
+            if (value < -1 || value >= kNumPairVariants) return fail(ctx, GG_ERR_ARG, "GG_OPT_PAIR_VARIANT: -1 or 0..%d", kNumPairVariants - 1);
             break;
         default:
             return fail(ctx, GG_ERR_UNSUPPORTED, "gg_set_option: unknown option %d", option);
@@ -653,8 +675,9 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
         case GG_OPT_GRAPH_CHUNK: ctx->opt_chunk = value; break;
         case GG_OPT_STREAM_VARIANT: ctx->opt_variant = (int)value; ctx->plan_ready = false; break;
         case GG_OPT_STREAM2_VARIANT: ctx->opt_variant2 = (int)value; ctx->plan2_ready = false; break;
-        case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = ctx->plan2_ready = false; break;
-        case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = ctx->plan2_ready = false; break;
+        case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = ctx->plan2_ready = false; ctx->pair.ready = false; break;
+        case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = ctx->plan2_ready = false; ctx->pair.ready = false; break;
+        case GG_OPT_PAIR_VARIANT: ctx->opt_pair_variant = (int)value; ctx->pair.ready = false; break;
     }
     return GG_OK;
 }
@@ -748,6 +771,7 @@ int gg_destroy(gg_ctx* ctx) {
 const char* gg_last_error(const gg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 int gg_num_stream_variants(void) { return kNumVariants; }
 int gg_num_stream2_variants(void) { return kNumVariants2; }
+int gg_num_pair_variants(void) { return kNumPairVariants; }
 const char* gg_version(void) { return "gg-b200 0.1 sm_100a"; }
 
 }  // extern "C"

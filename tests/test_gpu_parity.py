@@ -15,12 +15,12 @@ pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-10, "f32": 2e-4}
 KERNELS = {"generic": binding.GG_KERNEL_GENERIC, "stream": binding.GG_KERNEL_STREAM,
-           "stream2": binding.GG_KERNEL_STREAM2}
+           "stream2": binding.GG_KERNEL_STREAM2, "pair": binding.GG_KERNEL_PAIR}
 
 
 def expected_launches(kernel, calls):
     """Kernel launches for a list of gg_step(n) calls: stream2 advances two steps per launch."""
-    if kernel == "stream2":
+    if kernel in ("stream2", "pair"):
         return sum(n // 2 + n % 2 for n in calls)
     return sum(calls)
 
@@ -240,6 +240,60 @@ def test_rectangular_mesh_dx_ne_dy(ratio, dtype):
     # and the mesh ratio matters: the square-mesh result differs
     sq = workloads.random_problem(5, 328, 150, batch=2)
     assert np.max(np.abs(oracle_run(sq, 30)[2] - ref[2])) > 1e-6
+
+
+# ---------------------------------------------------------------------------------------------
+# GG_KERNEL_PAIR: two steps chained in registers, x-neighbours by warp shuffle
+# ---------------------------------------------------------------------------------------------
+def test_pair_every_variant_warps_and_chunking():
+    wl = workloads.random_problem(44, 488, 150, batch=2)   # fp64: 9 strips of 60 cells, ragged
+    ref = {n: oracle_run(wl, n) for n in (2, 5)}
+    base = {n: gpu_run(wl, n, kernel="stream")[0] for n in (2, 5)}
+    for v in range(binding.gg_num_pair_variants()):
+        for nw in (1, 3, 4, 5, 8):
+            for ipc, n in ((1, 2), (4, 5), (16, 2)):
+                try:
+                    got, used = gpu_run(wl, n, kernel="pair",
+                                        options=[(binding.GG_OPT_PAIR_VARIANT, v),
+                                                 (binding.GG_OPT_STREAM_WARPS, nw),
+                                                 (binding.GG_OPT_ITEMS_PER_WARP, ipc)])
+                except binding.GGError as e:
+                    assert e.code == binding.GG_ERR_UNSUPPORTED and "shared memory" in str(e)
+                    continue
+                assert used == "pair"
+                assert_close(got, ref[n], "f64", f"pair variant {v} warps {nw} items/CTA {ipc}")
+                for x, y in zip(got, base[n]):
+                    assert np.array_equal(x, y), f"pair variant {v} warps {nw}: not bit-identical"
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_pair_shapes_dtypes_and_boundaries(dtype):
+    for nx, ny, batch in ((4, 2, 1), (8, 3, 2), (60, 17, 1), (64, 64, 1), (124, 40, 3), (1000, 37, 1), (2056, 70, 1)):
+        wl = workloads.random_problem(300 + nx, nx, ny, batch=batch)
+        for n in (1, 2, 7):
+            got, used = gpu_run(wl, n, dtype=dtype, kernel="pair")
+            assert used == "pair"
+            assert_close(got, oracle_run(wl, n), dtype, f"pair {dtype} {nx}x{ny}x{batch} n={n}")
+
+
+def test_pair_configs_long_runs_bit_identical_to_single_step():
+    for wl, n in ((workloads.make(2, nx=520, ny=300, steps=200), 200),
+                  (workloads.make(3, nx=392, ny=250, steps=300), 301),
+                  (workloads.make(4, nx=264, ny=90, batch=5, steps=60), 60)):
+        a, _ = gpu_run(wl, n, kernel="pair", split=[1, 2, 3, 0, 7, n - 13])
+        b, _ = gpu_run(wl, n, kernel="stream")
+        for x, y in zip(a, b):
+            assert np.array_equal(x, y)
+        assert_close(a, oracle_run(wl, n), "f64", f"pair {wl.name}")
+    wl = workloads.make(3, nx=392, ny=250, steps=300)
+    got, _ = gpu_run(wl, 300, dtype="f32", kernel="pair")
+    assert_close(got, oracle_run(wl, 300), "f32", "pair cfg3 f32")
+
+
+def test_pair_rectangular_mesh():
+    wl = workloads.random_problem(6, 328, 150, batch=2, dy_ratio=0.6)
+    got, _ = gpu_run(wl, 30, kernel="pair")
+    assert_close(got, oracle_run(wl, 30), "f64", "pair dx != dy")
 
 
 def test_split_calls_equal_one_call():
