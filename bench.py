@@ -209,7 +209,12 @@ def run_ours(args, wl, rank, world, device):
     if args.kernel:
         sim.set_option(binding.GG_OPT_KERNEL, {"generic": binding.GG_KERNEL_GENERIC,
                                                "stream": binding.GG_KERNEL_STREAM,
-                                               "stream2": binding.GG_KERNEL_STREAM2}[args.kernel])
+                                               "stream2": binding.GG_KERNEL_STREAM2,
+                                               "pair": binding.GG_KERNEL_PAIR,
+                                               "quad": binding.GG_KERNEL_QUAD}[args.kernel])
+    for o, v in (("warps", binding.GG_OPT_STREAM_WARPS), ("variant", binding.GG_OPT_PAIR_VARIANT)):
+        if getattr(args, o) is not None:
+            sim.set_option(v, getattr(args, o))
     # pinned host copies of the inputs (what a host-side caller holds)
     host = {k: torch.from_numpy(np.ascontiguousarray(getattr(wl, k), dtype=npd)).pin_memory()
             for k in ("a", "b", "c", "U", "V", "W")}
@@ -292,7 +297,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--kernel", default=None, choices=[None, "generic", "stream", "stream2"])
+    ap.add_argument("--kernel", default=None, choices=[None, "generic", "stream", "stream2", "pair", "quad"])
+    ap.add_argument("--warps", type=int, default=None, help="tuning: GG_OPT_STREAM_WARPS")
+    ap.add_argument("--variant", type=int, default=None, help="tuning: GG_OPT_PAIR_VARIANT")
     ap.add_argument("--reps", type=int, default=3)
     ap.add_argument("--n", type=int, default=8192, help="grid edge (8192 = the headline config)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

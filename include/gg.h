@@ -69,8 +69,10 @@ enum {
                             /* needs nx*sizeof(elem) % 16 == 0                                  */
     GG_KERNEL_STREAM2 = 3,  /* as STREAM with two time steps fused per launch (temporal block)  */
     GG_KERNEL_RESIDENT = 4, /* whole state resident on-chip across steps (small grids; reserved)*/
-    GG_KERNEL_PAIR = 5      /* two time steps per launch chained in REGISTERS, x-neighbours by  */
+    GG_KERNEL_PAIR = 5,     /* two time steps per launch chained in REGISTERS, x-neighbours by  */
                             /* warp shuffle (gg_pair.cuh); needs nx*sizeof(elem) % 16 == 0      */
+    GG_KERNEL_QUAD = 6      /* FOUR time steps per launch: two register-chained pair marches    */
+                            /* linked by one shared-memory ring (gg_quad.cuh); same shape rule  */
 };
 enum {
     GG_OPT_KERNEL = 0,      /* one of GG_KERNEL_*                                               */
@@ -81,7 +83,8 @@ enum {
     GG_OPT_ITEMS_PER_WARP = 4,  /* tuning: target work items (row chunk x tile column) per resident CTA */
     GG_OPT_STREAM_WARPS = 5,    /* tuning: warps (= strips) per CTA: STREAM 1, 2, 4, 8; STREAM2 1, 2, 4; PAIR 1..8; 0 = from nx */
     GG_OPT_STREAM2_VARIANT = 6, /* tuning: build of the STREAM2 kernel, 0 .. gg_num_stream2_variants()-1; -1 = tuned default */
-    GG_OPT_PAIR_VARIANT = 7     /* tuning: build of the PAIR kernel, 0 .. gg_num_pair_variants()-1; -1 = deepest ring that fits */
+    GG_OPT_PAIR_VARIANT = 7,    /* tuning: build of the PAIR kernel, 0 .. gg_num_pair_variants()-1; -1 = deepest ring that fits */
+    GG_OPT_QUAD_VARIANT = 8     /* tuning: build of the QUAD kernel, 0 .. gg_num_quad_variants()-1; -1 = tuned default */
 };
 
 /* One simulation.  nx, ny >= 2 cells; h > 0 the mesh size (dx = dy = h);
@@ -188,6 +191,7 @@ const char* gg_last_error(const gg_ctx* ctx);
 int gg_num_stream_variants(void);
 int gg_num_stream2_variants(void);
 int gg_num_pair_variants(void);
+int gg_num_quad_variants(void);
 
 /* Library version string, e.g. "gg-b200 0.1 sm_100a". */
 const char* gg_version(void);

@@ -21,12 +21,12 @@ from . import build as _build
 GG_F64, GG_F32 = 0, 1
 GG_OK, GG_ERR_ARG, GG_ERR_STATE, GG_ERR_CUDA, GG_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
 GG_KERNEL_AUTO, GG_KERNEL_GENERIC, GG_KERNEL_STREAM, GG_KERNEL_STREAM2, GG_KERNEL_RESIDENT, \
-    GG_KERNEL_PAIR = range(6)
+    GG_KERNEL_PAIR, GG_KERNEL_QUAD = range(7)
 GG_OPT_KERNEL, GG_OPT_GRAPH, GG_OPT_GRAPH_CHUNK, GG_OPT_STREAM_VARIANT, GG_OPT_ITEMS_PER_WARP, \
-    GG_OPT_STREAM_WARPS, GG_OPT_STREAM2_VARIANT, GG_OPT_PAIR_VARIANT = range(8)
+    GG_OPT_STREAM_WARPS, GG_OPT_STREAM2_VARIANT, GG_OPT_PAIR_VARIANT, GG_OPT_QUAD_VARIANT = range(9)
 
 KERNEL_NAMES = {GG_KERNEL_AUTO: "auto", GG_KERNEL_GENERIC: "generic", GG_KERNEL_STREAM: "stream",
-                GG_KERNEL_STREAM2: "stream2", GG_KERNEL_RESIDENT: "resident", GG_KERNEL_PAIR: "pair"}
+                GG_KERNEL_STREAM2: "stream2", GG_KERNEL_RESIDENT: "resident", GG_KERNEL_PAIR: "pair", GG_KERNEL_QUAD: "quad"}
 
 _vp = ctypes.c_void_p
 _dp = ctypes.POINTER(ctypes.c_double)
@@ -62,6 +62,7 @@ SIGNATURES = {
     "gg_num_stream_variants": (ctypes.c_int, []),
     "gg_num_stream2_variants": (ctypes.c_int, []),
     "gg_num_pair_variants": (ctypes.c_int, []),
+    "gg_num_quad_variants": (ctypes.c_int, []),
     "gg_version": (ctypes.c_char_p, []),
 }
 
@@ -217,6 +218,10 @@ def gg_num_stream2_variants() -> int:
 
 def gg_num_pair_variants() -> int:
     return int(load().gg_num_pair_variants())
+
+
+def gg_num_quad_variants() -> int:
+    return int(load().gg_num_quad_variants())
 
 
 # ---- convenience holder (torch owns device memory and the stream) ------------------------------

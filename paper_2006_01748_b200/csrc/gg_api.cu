@@ -22,6 +22,7 @@
 #include "gg_stream2.cuh"
 #include "gg_diag.cuh"
 #include "gg_pair.cuh"
+#include "gg_quad.cuh"
 
 namespace {
 
@@ -74,8 +75,8 @@ struct gg_ctx {
         size_t smem = 0;
         const void* fn = nullptr;
         bool ready = false;
-    } pair;
-    int opt_pair_variant = -1;
+    } pair, quad;
+    int opt_pair_variant = -1, opt_quad_variant = -1;
     int opt_variant2 = -1;        // -1 = tuned default for the dtype
     // graphs
     std::map<GraphKey, cudaGraphExec_t> graphs;
@@ -271,7 +272,7 @@ int build_plan(gg_ctx* c, bool two_step) {
     const int strip_cells = gg::kStripBytes / (int)c->esize();
     const int nstrips = (c->nx + strip_cells - 1) / strip_cells;
     int nw = c->opt_warps;
-    if (resolve_kernel(c) == GG_KERNEL_PAIR) nw = 0;  // GG_OPT_STREAM_WARPS then addresses the pair kernel
+    if (resolve_kernel(c) == GG_KERNEL_PAIR || resolve_kernel(c) == GG_KERNEL_QUAD) nw = 0;  // GG_OPT_STREAM_WARPS then addresses the pair kernel
     // Tuned on B200 at 8192^2: fp64 runs 4 rows per box with 4 strips per
     // step; fp32 runs 3 rows per box with 2 strips (its row body is twice as long per lane, and
     // the smaller build keeps the three warp roles inside the instruction cache).
@@ -412,8 +413,9 @@ int enqueue_steps(gg_ctx* c, int kernel, int src, long long len, double dt, long
     while (len > 0) {
         int rc;
         if (kernel == GG_KERNEL_STREAM2 && len >= 2) { rc = launch_stream(c, s, dt, true); len -= 2; }
-        else if (kernel == GG_KERNEL_PAIR && len >= 2) { rc = launch_pair(c, s, dt); len -= 2; }
-        else if (kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR) { rc = launch_stream(c, s, dt, false); len -= 1; }
+        else if (kernel == GG_KERNEL_QUAD && len >= 4) { rc = launch_multi(c, c->quad, s, dt); len -= 4; }
+        else if ((kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) && len >= 2) { rc = launch_pair(c, s, dt); len -= 2; }
+        else if (kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) { rc = launch_stream(c, s, dt, false); len -= 1; }
         else { rc = launch_step(c, kernel, s, dt); len -= 1; }
         if (rc) return rc;
         s ^= 1;
@@ -585,12 +587,17 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
     if (n == 0) return GG_OK;
     const int kernel = resolve_kernel(ctx);
-    if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR) {
+    if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ||
+        kernel == GG_KERNEL_QUAD) {
         int rc = build_plan(ctx, false);
         if (rc) return rc;
     }
-    if (kernel == GG_KERNEL_PAIR) {
+    if (kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) {
         int rc = build_plan_pair(ctx);
+        if (rc) return rc;
+    }
+    if (kernel == GG_KERNEL_QUAD) {
+        int rc = build_plan_quad(ctx);
         if (rc) return rc;
     }
     if (kernel == GG_KERNEL_STREAM2) {
@@ -598,6 +605,7 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
         if (rc) return rc;
     }
     auto launches_for = [kernel](long long len) {
+        if (kernel == GG_KERNEL_QUAD) return len / 4 + ((len % 4) >> 1) + (len & 1);
         return kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ? len / 2 + (len & 1) : len;
     };
     GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
@@ -637,7 +645,8 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
     switch (option) {
         case GG_OPT_KERNEL:
             if (value == GG_KERNEL_AUTO || value == GG_KERNEL_GENERIC) break;
-            if (value == GG_KERNEL_STREAM || value == GG_KERNEL_STREAM2 || value == GG_KERNEL_PAIR) {
+            if (value == GG_KERNEL_STREAM || value == GG_KERNEL_STREAM2 || value == GG_KERNEL_PAIR ||
+                value == GG_KERNEL_QUAD) {
                 if (!stream_shape_ok(ctx))
                     return fail(ctx, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0 (nx = %d)", ctx->nx);
                 break;
@@ -662,6 +671,9 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
             if (value < 0 || value > 8)
                 return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_WARPS: 0..8");
             break;
+        case GG_OPT_QUAD_VARIANT:
+            if (value < -1 || value >= kNumQuadVariants) return fail(ctx, GG_ERR_ARG, "GG_OPT_QUAD_VARIANT: -1 or 0..%d", kNumQuadVariants - 1);
+            break;
         case GG_OPT_PAIR_VARIANT:
             if (value < -1 || value >= kNumPairVariants) return fail(ctx, GG_ERR_ARG, "GG_OPT_PAIR_VARIANT: -1 or 0..%d", kNumPairVariants - 1);
             break;
@@ -675,9 +687,10 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
         case GG_OPT_GRAPH_CHUNK: ctx->opt_chunk = value; break;
         case GG_OPT_STREAM_VARIANT: ctx->opt_variant = (int)value; ctx->plan_ready = false; break;
         case GG_OPT_STREAM2_VARIANT: ctx->opt_variant2 = (int)value; ctx->plan2_ready = false; break;
-        case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = ctx->plan2_ready = false; ctx->pair.ready = false; break;
+        case GG_OPT_ITEMS_PER_WARP: ctx->opt_items_per_warp = (int)value; ctx->plan_ready = ctx->plan2_ready = false; ctx->pair.ready = ctx->quad.ready = false; break;
         case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = ctx->plan2_ready = false; ctx->pair.ready = false; break;
         case GG_OPT_PAIR_VARIANT: ctx->opt_pair_variant = (int)value; ctx->pair.ready = false; break;
+        case GG_OPT_QUAD_VARIANT: ctx->opt_quad_variant = (int)value; ctx->quad.ready = false; break;
     }
     return GG_OK;
 }
@@ -772,6 +785,7 @@ const char* gg_last_error(const gg_ctx* ctx) { return ctx ? ctx->err.c_str() : g
 int gg_num_stream_variants(void) { return kNumVariants; }
 int gg_num_stream2_variants(void) { return kNumVariants2; }
 int gg_num_pair_variants(void) { return kNumPairVariants; }
+int gg_num_quad_variants(void) { return kNumQuadVariants; }
 const char* gg_version(void) { return "gg-b200 0.1 sm_100a"; }
 
 }  // extern "C"

@@ -1,0 +1,224 @@
+// gg_quad.cuh -- GG_KERNEL_QUAD: FOUR time steps per launch.
+//
+// The register-chained pair kernel (gg_pair.cuh) runs at the HBM rate with the SM ~45 % busy
+// (profiles/r01_ncu_full_pair_f64.txt), so the remaining headroom is again in crossing HBM less
+// often.  Two pair marches are chained through one shared-memory ring:
+//
+//   TMA --ring0: U,V,W,a,b,c at time k--> 4 "A" warps: k -> k+1 -> k+2 in registers
+//       --ring1: U,V,W at time k+2 (+ the rows' a,b,c)--> 4 "B" warps: k+2 -> k+3 -> k+4 --> HBM
+//
+//  * Geometry in units of lane runs (one run = C cells = 16 bytes).  A pair march loses one lane
+//    on each side of a warp, and a lane's result depends on its own and its two neighbours'
+//    inputs only.  A warp w lane l owns run 30w-2+l of the tile and leaves 120 valid time-k+2
+//    runs [-1, 119) in ring1; B warp w lane l owns run 30w-1+l; the tile's time-k+4 output is
+//    runs [0, 118): 118 x 16 B = 1888 contiguous bytes per row and field.  Work per output
+//    cell-step: 8 x 32 lanes x 2 levels / (118 x 4) = 1.085 lane-rows (1.067 in the pair kernel).
+//  * ring0 is the pair kernel's ring for four warps (TMA boxes of GW strips + overlap); a slot is
+//    refilled by the A warp that releases it last.  ring1 rows are contiguous (123 runs).  A
+//    writes lanes 1..30; B's outermost lanes read two runs nobody writes (zeroed at start-up) and
+//    produce nothing that is kept.  mbarriers: full0 (TMA bytes), full1 (4 A warps), empty1 (4 B
+//    warps); no __syncthreads after start-up.
+//  * Rows: a chunk [j0, j1) loads rows j0-4 .. j1+3; A emits time-k+2 rows j0-2 .. j1+1; B stores
+//    time-k+4 rows j0 .. j1-1.
+//  * Both roles run the SAME row body (PairLevel twice); they differ in where a row comes from and
+//    where the result goes.  Arithmetic and operand order are every other kernel's => bit-identical.
+#pragma once
+#include "gg_pair.cuh"
+
+namespace gg {
+
+constexpr int kQuadRuns = 118;         // output runs per tile row
+constexpr int kQuadRing1Runs = 123;    // runs per ring1 row (run -2 .. 120)
+
+template <typename T> __host__ __device__ constexpr int quad_ring0_stage(int rb) {
+    return 6 * (4 / pair_gw<T>()) * pair_slab_bytes(rb, pair_box_bytes<T>());
+}
+__host__ __device__ constexpr int quad_ring1_stage(int rb) { return 6 * rb * kQuadRing1Runs * 16; }
+template <typename T> __host__ __device__ constexpr int quad_smem_bytes(int rb, int nst0, int nst1) {
+    return 256 + nst0 * quad_ring0_stage<T>(rb) + nst1 * quad_ring1_stage(rb);
+}
+
+template <int RB>
+__device__ __forceinline__ PairItem quad_item(const PairArgs& A, long long item, int tile_cells) {
+    PairItem it = pair_item<RB>(A, item, tile_cells);
+    it.nr = it.j1 - it.j0 + 8;  // time-k rows j0-4 .. j1+3 arrive
+    it.nstage = (it.nr + RB - 1) / RB;
+    return it;
+}
+
+// blockDim = 256: warps 0..3 = A, 4..7 = B.  Dynamic shared memory:
+// [full0[NST0], full1[NST1], empty1[NST1] mbarriers, count0[NST0]; 256 B][ring0][ring1].
+template <typename T, int RB, int NST0, int NST1>
+__global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ PairArgs A) {
+    constexpr int C = 16 / (int)sizeof(T);
+    constexpr int GW = pair_gw<T>();
+    constexpr int NG = 4 / GW;
+    constexpr int VW = kPairLanes * C;
+    constexpr int BOXB = pair_box_bytes<T>();
+    constexpr int SLAB = pair_slab_bytes(RB, BOXB);
+    constexpr int ARR0 = NG * SLAB, STAGE0 = 6 * ARR0;
+    constexpr int P1 = kQuadRing1Runs * 16, ARR1 = RB * P1, STAGE1 = 6 * ARR1;
+    static_assert(STAGE0 == quad_ring0_stage<T>(RB) && STAGE1 == quad_ring1_stage(RB), "layout");
+    static_assert((NST0 + 2 * NST1) * 8 + NST0 * 4 <= 256, "too many stages");
+
+    extern __shared__ __align__(128) char smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool isA = warp < 4;
+    const int w = warp & 3;
+    const uint32_t full0 = smem_u32(smem), full1 = full0 + 8u * NST0, empty1 = full1 + 8u * NST1;
+    unsigned int* count0 = reinterpret_cast<unsigned int*>(smem + 8 * (NST0 + 2 * NST1));
+    char* ring0 = smem + 256;
+    char* ring1 = ring0 + (size_t)NST0 * STAGE0;
+    const uint32_t ring0_u32 = smem_u32(ring0);
+    const int nx = A.nx, ny = A.ny;
+    const int tile_cells = kQuadRuns * C;
+    constexpr int NBOX = 6 * NG;
+    constexpr uint32_t STAGE_TX = (uint32_t)(NBOX * RB * BOXB);
+
+    auto issue = [&](const PairCursor& pc, uint32_t slot) {
+        const uint32_t bar = full0 + 8u * slot;
+        const uint32_t dst = ring0_u32 + slot * STAGE0;
+        const int y = pc.it.j0 - 4 + pc.q * RB;
+        if (lane == 0) mbar_expect_tx(bar, STAGE_TX);
+        __syncwarp();
+        if (lane < NBOX) {
+            const int f = lane / NG, g = lane - NG * f;
+            const CUtensorMap* map = f == 0 ? &A.mU : f == 1 ? &A.mV : f == 2 ? &A.mW
+                                   : f == 3 ? &A.ma : f == 4 ? &A.mb : &A.mc;
+            tma_load_3d(dst + f * ARR0 + g * SLAB, map, bar, pc.it.i0 - 2 * C + g * GW * VW, y,
+                        f < 3 ? pc.it.sim : 0);
+        }
+    };
+    auto advance_cursor = [&](PairCursor& pc) {
+        if (pc.item >= A.nitems) return;
+        if (++pc.q == pc.it.nstage) {
+            pc.q = 0;
+            pc.item += gridDim.x;
+            if (pc.item < A.nitems) pc.it = quad_item<RB>(A, pc.item, tile_cells);
+        }
+    };
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST0; ++s) { mbar_init(full0 + 8u * s, 1); count0[s] = 0u; }
+        for (int s = 0; s < NST1; ++s) { mbar_init(full1 + 8u * s, 4); mbar_init(empty1 + 8u * s, 4); }
+        fence_barrier_init();
+        fence_proxy_async();
+    }
+    // ring1 runs that no A lane writes are read (and discarded) by B's outermost lanes
+    for (int o = threadIdx.x * 16; o < NST1 * STAGE1; o += 256 * 16)
+        *reinterpret_cast<uint4*>(ring1 + o) = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
+
+    PairCursor pc;
+    pc.item = blockIdx.x;
+    pc.q = 0;
+    if (pc.item < A.nitems) pc.it = quad_item<RB>(A, pc.item, tile_cells);
+    if (isA) {
+        for (int s = 0; s < NST0; ++s) {
+            if (warp == 0 && pc.item < A.nitems) issue(pc, (uint32_t)s);
+            advance_cursor(pc);
+        }
+    }
+
+    // where this lane finds its run in a stage of its source ring, and the ring's strides
+    const int src_off = isA ? (w / GW) * SLAB + (w % GW) * (VW * (int)sizeof(T)) + 16 * lane
+                            : (30 * w + lane + 1) * 16;
+    const int src_arr = isA ? ARR0 : ARR1, src_row = isA ? BOXB : P1;
+    const int dst_off = (30 * w + lane) * 16;              // A: own run in a ring1 row
+    const int run0 = isA ? 30 * w - 2 + lane : 30 * w - 1 + lane;  // tile run this lane owns
+    const bool lane_ok = lane >= 1 && lane <= (isA || w < 3 ? kPairLanes : kPairLanes - 2);
+    const size_t plane = (size_t)nx * ny;
+
+    uint32_t gc = 0;
+    for (long long item = blockIdx.x; item < A.nitems; item += gridDim.x) {
+        const PairItem it = quad_item<RB>(A, item, tile_cells);
+        const int iown = it.i0 + run0 * C;               // first own cell (may lie outside the domain)
+        const bool store_ok = lane_ok && iown >= 0 && iown < nx;
+        const bool atW = iown == 0, atE = iown + C == nx;
+        const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+        T* gU = (T*)A.U1 + it.sim * plane + iown;
+        T* gV = (T*)A.V1 + it.sim * plane + iown;
+        T* gW = (T*)A.W1 + it.sim * plane + iown;
+
+        PairLevel<T, C> L1, L2;
+        L1.clear();
+        L2.clear();
+
+        for (int q = 0; q < it.nstage; ++q, ++gc) {
+            const uint32_t s0 = gc % NST0, s1 = gc % NST1;
+            if (isA) {
+                mbar_wait(full0 + 8u * s0, (gc / NST0) & 1u);
+                if (gc >= NST1) mbar_wait(empty1 + 8u * s1, ((gc / NST1) - 1u) & 1u);
+            } else {
+                mbar_wait(full1 + 8u * s1, (gc / NST1) & 1u);
+            }
+            const char* src = (isA ? ring0 + (size_t)s0 * STAGE0 : ring1 + (size_t)s1 * STAGE1) + src_off;
+            char* dst = ring1 + (size_t)s1 * STAGE1 + dst_off;
+            // first row arriving at this role in this stage: time k for A, time k+2 for B
+            const int jfirst = it.j0 - 4 + q * RB - (isA ? 0 : 2);
+            auto row_body = [&](auto ghost_c, const int rr) {
+                constexpr bool GHOST = decltype(ghost_c)::value;
+                const int jn = jfirst + rr;
+                const char* p = src + rr * src_row;
+                T uN[C], vN[C], wN[C], aN[C], bN[C], cN[C];
+                ld_run<T, C>(p + 0 * src_arr, uN);
+                ld_run<T, C>(p + 1 * src_arr, vN);
+                ld_run<T, C>(p + 2 * src_arr, wN);
+                ld_run<T, C>(p + 3 * src_arr, aN);
+                ld_run<T, C>(p + 4 * src_arr, bN);
+                ld_run<T, C>(p + 5 * src_arr, cN);
+                T u1[C], v1[C], w1[C], a1[C], b1[C], c1[C];   // row jn-1, one level up
+                L1.template advance<GHOST>(jn, ny, atW, atE, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
+                T u2[C], v2[C], w2[C], a2[C], b2[C], c2[C];   // row jn-2, two levels up
+                L2.template advance<GHOST>(jn - 1, ny, atW, atE, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
+                if (isA) {
+                    if (lane_ok) {                            // time-k+2 row jn-2 and its coefficients
+                        char* o = dst + rr * P1;
+                        st_run<T, C>(o + 0 * ARR1, u2);
+                        st_run<T, C>(o + 1 * ARR1, v2);
+                        st_run<T, C>(o + 2 * ARR1, w2);
+                        st_run<T, C>(o + 3 * ARR1, a2);
+                        st_run<T, C>(o + 4 * ARR1, b2);
+                        st_run<T, C>(o + 5 * ARR1, c2);
+                    }
+                } else {
+                    const int r = jn - 2;                     // time-k+4 row
+                    if (store_ok && r >= it.j0 && r < it.j1) {
+                        const size_t off = (size_t)r * nx;
+                        st_run<T, C>((char*)(gU + off), u2);
+                        st_run<T, C>((char*)(gV + off), v2);
+                        st_run<T, C>((char*)(gW + off), w2);
+                    }
+                }
+            };
+            if (jfirst >= 2 && jfirst + RB - 1 < ny) {
+#pragma unroll
+                for (int rr = 0; rr < RB; ++rr) row_body(std::false_type{}, rr);
+            } else {
+#pragma unroll
+                for (int rr = 0; rr < RB; ++rr) row_body(std::true_type{}, rr);
+            }
+            __syncwarp();
+            if (isA) {
+                // ring1 stage written (release); ring0 slot read: the A warp that releases it last
+                // refills it with the stage NST0 ahead
+                unsigned int prev = 0;
+                if (lane == 0) {
+                    mbar_arrive(full1 + 8u * s1);
+                    __threadfence_block();
+                    prev = atomicAdd(&count0[s0], 1u);
+                }
+                prev = __shfl_sync(0xffffffffu, prev, 0);
+                if (prev == 3u) {
+                    if (lane == 0) { count0[s0] = 0u; __threadfence_block(); }
+                    if (pc.item < A.nitems) issue(pc, s0);
+                }
+                advance_cursor(pc);
+            } else if (lane == 0) {
+                mbar_arrive(empty1 + 8u * s1);
+            }
+        }
+    }
+}
+
+}  // namespace gg

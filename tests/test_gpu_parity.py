@@ -15,11 +15,14 @@ pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-10, "f32": 2e-4}
 KERNELS = {"generic": binding.GG_KERNEL_GENERIC, "stream": binding.GG_KERNEL_STREAM,
-           "stream2": binding.GG_KERNEL_STREAM2, "pair": binding.GG_KERNEL_PAIR}
+           "stream2": binding.GG_KERNEL_STREAM2, "pair": binding.GG_KERNEL_PAIR,
+           "quad": binding.GG_KERNEL_QUAD}
 
 
 def expected_launches(kernel, calls):
     """Kernel launches for a list of gg_step(n) calls: stream2 advances two steps per launch."""
+    if kernel == "quad":
+        return sum(n // 4 + (n % 4) // 2 + n % 2 for n in calls)
     if kernel in ("stream2", "pair"):
         return sum(n // 2 + n % 2 for n in calls)
     return sum(calls)
@@ -294,6 +297,51 @@ def test_pair_rectangular_mesh():
     wl = workloads.random_problem(6, 328, 150, batch=2, dy_ratio=0.6)
     got, _ = gpu_run(wl, 30, kernel="pair")
     assert_close(got, oracle_run(wl, 30), "f64", "pair dx != dy")
+
+
+# ---------------------------------------------------------------------------------------------
+# GG_KERNEL_QUAD: four steps per launch (two register-chained pair marches linked by a ring)
+# ---------------------------------------------------------------------------------------------
+def test_quad_every_variant_and_chunking():
+    wl = workloads.random_problem(45, 488, 150, batch=2)   # fp64: 3 tiles of 236 cells, ragged
+    ref = {n: oracle_run(wl, n) for n in (4, 11)}
+    base = {n: gpu_run(wl, n, kernel="stream")[0] for n in (4, 11)}
+    for v in range(binding.gg_num_quad_variants()):
+        for ipc, n in ((1, 4), (4, 11), (16, 4)):
+            got, used = gpu_run(wl, n, kernel="quad", options=[(binding.GG_OPT_QUAD_VARIANT, v),
+                                                               (binding.GG_OPT_ITEMS_PER_WARP, ipc)])
+            assert used == "quad"
+            assert_close(got, ref[n], "f64", f"quad variant {v} items/CTA {ipc}")
+            for x, y in zip(got, base[n]):
+                assert np.array_equal(x, y), f"quad variant {v}: not bit-identical"
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_quad_shapes_dtypes_and_boundaries(dtype):
+    for nx, ny, batch in ((4, 2, 1), (8, 3, 2), (60, 17, 1), (236, 64, 1), (240, 40, 3), (472, 9, 1),
+                          (1000, 37, 1), (2056, 70, 1)):
+        wl = workloads.random_problem(400 + nx, nx, ny, batch=batch)
+        for n in (4, 7, 8):
+            got, used = gpu_run(wl, n, dtype=dtype, kernel="quad")
+            assert used == "quad"
+            assert_close(got, oracle_run(wl, n), dtype, f"quad {dtype} {nx}x{ny}x{batch} n={n}")
+
+
+def test_quad_configs_long_runs_bit_identical_to_single_step():
+    for wl, n in ((workloads.make(2, nx=520, ny=300, steps=200), 200),
+                  (workloads.make(3, nx=392, ny=250, steps=300), 303),
+                  (workloads.make(4, nx=264, ny=90, batch=5, steps=60), 60)):
+        a, _ = gpu_run(wl, n, kernel="quad", split=[1, 2, 3, 0, 7, n - 13])
+        b, _ = gpu_run(wl, n, kernel="stream")
+        for x, y in zip(a, b):
+            assert np.array_equal(x, y)
+        assert_close(a, oracle_run(wl, n), "f64", f"quad {wl.name}")
+    wl = workloads.make(3, nx=392, ny=250, steps=300)
+    got, _ = gpu_run(wl, 300, dtype="f32", kernel="quad")
+    assert_close(got, oracle_run(wl, 300), "f32", "quad cfg3 f32")
+    wl = workloads.random_problem(7, 328, 150, batch=2, dy_ratio=0.6)
+    got, _ = gpu_run(wl, 32, kernel="quad")
+    assert_close(got, oracle_run(wl, 32), "f64", "quad dx != dy")
 
 
 def test_split_calls_equal_one_call():
