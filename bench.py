@@ -366,7 +366,7 @@ def main():
         line["parity_sample_max_abs_err"] = sampled_parity(wl, res["final"], args.steps)
         log(f"sampled parity: {line['parity_sample_max_abs_err']:.3e} ({time.perf_counter() - t0:.1f} s)")
         if not args.no_cpu and world == 1:
-            g, desc, cores, _ = oracle_sample(wl, rows=1024, steps=20)
+            g, desc, cores, _ = oracle_sample(wl, rows=2048, steps=200)
             line["cpu_baseline"] = {"value": g, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": desc}
         print(json.dumps(line), flush=True)

@@ -83,7 +83,7 @@ enum {
     GG_OPT_ITEMS_PER_WARP = 4,  /* tuning: target work items (row chunk x tile column) per resident CTA */
     GG_OPT_STREAM_WARPS = 5,    /* tuning: warps (= strips) per CTA: STREAM 1, 2, 4, 8; STREAM2 1, 2, 4; PAIR 1..8; 0 = from nx */
     GG_OPT_STREAM2_VARIANT = 6, /* tuning: build of the STREAM2 kernel, 0 .. gg_num_stream2_variants()-1; -1 = tuned default */
-    GG_OPT_PAIR_VARIANT = 7,    /* tuning: build of the PAIR kernel, 0 .. gg_num_pair_variants()-1; -1 = deepest ring that fits */
+    GG_OPT_PAIR_VARIANT = 7,    /* tuning: build of the PAIR kernel, 0 .. gg_num_pair_variants()-1; -1 = tuned default */
     GG_OPT_QUAD_VARIANT = 8     /* tuning: build of the QUAD kernel, 0 .. gg_num_quad_variants()-1; -1 = tuned default */
 };
 

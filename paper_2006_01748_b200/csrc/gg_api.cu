@@ -141,7 +141,13 @@ bool stream_shape_ok(const gg_ctx* c) { return ((size_t)c->nx * c->esize()) % 16
 
 int resolve_kernel(const gg_ctx* c) {
     if (c->opt_kernel != GG_KERNEL_AUTO) return c->opt_kernel;
-    return stream_shape_ok(c) ? GG_KERNEL_STREAM2 : GG_KERNEL_GENERIC;
+    if (!stream_shape_ok(c)) return GG_KERNEL_GENERIC;
+    // Tuned on B200.  The deeper the temporal blocking, the larger the
+    // per-launch pipeline fill and the halo overhead, so small grids stay with shallower kernels.
+    const double cells = (double)c->nx * c->ny * c->nbatch;
+    if (c->dtype == GG_F64 && c->nx >= 4096 && cells >= 16777216.0) return GG_KERNEL_QUAD;
+    if (cells > 262144.0 && c->nx >= 240) return GG_KERNEL_PAIR;
+    return GG_KERNEL_STREAM2;
 }
 
 void drop_graphs(gg_ctx* c) {

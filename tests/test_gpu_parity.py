@@ -73,7 +73,7 @@ def test_config0_full(kernel):
 def test_config1_full():
     wl = workloads.make(1)
     got, used = gpu_run(wl, wl.steps)
-    assert used == "stream2"   # AUTO
+    assert used == "stream2"   # AUTO: a 512^2 grid is launch-latency bound; two steps per launch
     ref = oracle_run(wl, wl.steps)
     assert_close(got, ref, "f64", "cfg1")
 
