@@ -362,6 +362,20 @@ def main():
                          "frac_of_nominal_8000": achieved / 8000.0},
             "e2e": res["e2e"], "gpu_launches": res["launches"], "clocks": res["clocks"],
         }
+        # The multi-step kernels are no longer HBM-bound (ncu: DRAM 3.8 TB/s for `quad`); their
+        # nearest ceiling is the plain-ALU pipe of the arithmetic type.  Thread instructions per
+        # cell-step from the ncu captures (fp64 / fp32 pipe instructions x 32 / cell-steps of the
+        # launch, redundant overlap lanes included); peak = 148 SMs x lanes per clock x the max SM
+        # clock (one fused multiply-add = one instruction), DESIGN.md section 8.
+        ops = {"quad": 43.0, "pair": 42.5, "stream2": 52.0, "stream": 52.0}.get(res["kernel"])
+        if ops is not None:
+            lanes = 64 if args.dtype == "f64" else 128
+            mhz = (res["clocks"] or {}).get("sm_max_mhz") or 1965.0
+            alu_peak = 148 * lanes * mhz * 1e6 / 1e12
+            alu = res["value"] * 1e9 * ops / 1e12
+            line["alu"] = {"bound": "alu", "achieved": alu, "peak": alu_peak,
+                           "unit": f"T {args.dtype} instr/s", "frac": alu / alu_peak,
+                           "instr_per_cell_step": ops}
         t0 = time.perf_counter()
         line["parity_sample_max_abs_err"] = sampled_parity(wl, res["final"], args.steps)
         log(f"sampled parity: {line['parity_sample_max_abs_err']:.3e} ({time.perf_counter() - t0:.1f} s)")
