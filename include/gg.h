@@ -68,7 +68,10 @@ enum {
     GG_KERNEL_STREAM = 2,   /* TMA-staged shared-memory row ring, register-rolling y march;     */
                             /* needs nx*sizeof(elem) % 16 == 0                                  */
     GG_KERNEL_STREAM2 = 3,  /* as STREAM with two time steps fused per launch (temporal block)  */
-    GG_KERNEL_RESIDENT = 4, /* whole state resident on-chip across steps (small grids; reserved)*/
+    GG_KERNEL_RESIDENT = 4, /* all n steps of a call in ONE cooperative launch, state resident in */
+                            /* shared memory, row slabs exchange edge rows point-to-point; grids */
+                            /* of at most 148 slabs with rows <= 4096 B (gg_resident.cuh).  AUTO  */
+                            /* uses it for calls of >= 8 steps and STREAM2 for shorter ones       */
     GG_KERNEL_PAIR = 5,     /* two time steps per launch chained in REGISTERS, x-neighbours by  */
                             /* warp shuffle (gg_pair.cuh); needs nx*sizeof(elem) % 16 == 0      */
     GG_KERNEL_QUAD = 6      /* FOUR time steps per launch: two register-chained pair marches    */
@@ -171,7 +174,8 @@ int gg_set_option(gg_ctx* ctx, int option, long long value);
 /* Introspection for benchmarks and tests.
  * gg_kernel_used: GG_KERNEL_* the next gg_step will run (resolves AUTO), or -1.
  * gg_launches:    number of step kernels this context has launched so far (graph replays count
- *                 every kernel node; a GG_KERNEL_STREAM2 launch advances two steps).
+ *                 every kernel node; a STREAM2 / PAIR launch advances two steps, a QUAD launch
+ *                 four, a RESIDENT launch all n steps of its gg_step call).
  * gg_last_step_ms: device time of the most recent gg_step call, measured with CUDA events
  *                 recorded on the bound stream around its launches; synchronises on the end
  *                 event.  *ms < 0 if no step has run. */

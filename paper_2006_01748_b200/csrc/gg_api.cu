@@ -23,6 +23,7 @@
 #include "gg_diag.cuh"
 #include "gg_pair.cuh"
 #include "gg_quad.cuh"
+#include "gg_resident.cuh"
 
 namespace {
 
@@ -77,6 +78,15 @@ struct gg_ctx {
         bool ready = false;
     } pair, quad;
     int opt_pair_variant = -1, opt_quad_variant = -1;
+    // on-chip resident kernel (gg_resident.cuh)
+    struct ResidentPlan {
+        int R = 0, slabs_per_sim = 0, grid = 0, block = 0;
+        size_t smem = 0;
+        const void* fn = nullptr;
+        bool ready = false;
+    } resident;
+    void* d_res_halo = nullptr;
+    unsigned int* d_res_flags = nullptr;
     int opt_variant2 = -1;        // -1 = tuned default for the dtype
     // graphs
     std::map<GraphKey, cudaGraphExec_t> graphs;
@@ -112,8 +122,10 @@ int fail(const gg_ctx* c, int code, const char* fmt, ...) {
     } while (0)
 
 struct Layout {
-    size_t state[2][3], coef[3], sims, scratch, total;
+    size_t state[2][3], coef[3], sims, scratch, res_halo, res_flags, total;
 };
+int resident_rows(const gg_ctx* c, int max_slabs);
+size_t resident_halo_bytes(const gg_ctx* c);
 // scratch for the reductions of gg_diag.cuh: [nbatch][kDiagMaxBlocks][8] partials + [nbatch][8]
 size_t scratch_doubles(const gg_ctx* c);
 
@@ -129,6 +141,14 @@ Layout layout_of(const gg_ctx* c) {
     off += align_up((size_t)c->nbatch * sizeof(gg::SimScalars));
     L.scratch = off;
     off += align_up(scratch_doubles(c) * sizeof(double));
+    // edge-row exchange buffers and step counters of the resident kernel (small grids only)
+    L.res_halo = L.res_flags = 0;
+    if (resident_rows(c, 148) > 0) {
+        L.res_halo = off;
+        off += align_up(resident_halo_bytes(c));
+        L.res_flags = off;
+        off += align_up(148 * sizeof(unsigned int));
+    }
     L.total = off;
     return L;
 }
@@ -145,6 +165,9 @@ int resolve_kernel(const gg_ctx* c) {
     // Tuned on B200.  The deeper the temporal blocking, the larger the
     // per-launch pipeline fill and the halo overhead, so small grids stay with shallower kernels.
     const double cells = (double)c->nx * c->ny * c->nbatch;
+    // grids that fit on chip: one cooperative launch for the whole call (gg_step uses it for
+    // calls of at least kResidentMinSteps steps and STREAM2 for shorter ones)
+    if (resident_rows(c, c->bound ? (c->num_sms < 148 ? c->num_sms : 148) : 148) > 0) return GG_KERNEL_RESIDENT;
     if (c->dtype == GG_F64 && c->nx >= 4096 && cells >= 16777216.0) return GG_KERNEL_QUAD;
     if (cells > 262144.0 && c->nx >= 240) return GG_KERNEL_PAIR;
     return GG_KERNEL_STREAM2;
@@ -361,6 +384,7 @@ int build_plan(gg_ctx* c, bool two_step) {
 }
 
 #include "gg_pair_plan.inc"
+#include "gg_resident_plan.inc"
 
 template <typename T>
 int launch_generic(gg_ctx* c, int src, double dt) {
@@ -494,6 +518,10 @@ int gg_bind(gg_ctx* ctx, void* ws, size_t bytes, void* stream) {
     for (int f = 0; f < 3; ++f) ctx->coef[f] = ctx->ws + L.coef[f];
     ctx->d_sims = (gg::SimScalars*)(ctx->ws + L.sims);
     ctx->d_scratch = (double*)(ctx->ws + L.scratch);
+    if (L.res_halo) {
+        ctx->d_res_halo = ctx->ws + L.res_halo;
+        ctx->d_res_flags = (unsigned int*)(ctx->ws + L.res_flags);
+    }
     GG_CUDA(ctx, cudaMemcpyAsync(ctx->d_sims, ctx->sims.data(), ctx->sims.size() * sizeof(gg::SimScalars),
                                  cudaMemcpyHostToDevice, ctx->stream));
     GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // sims is pageable host memory
@@ -592,7 +620,21 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
     if (n < 0) return fail(ctx, GG_ERR_ARG, "gg_step: n = %lld < 0", n);
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
     if (n == 0) return GG_OK;
-    const int kernel = resolve_kernel(ctx);
+    int kernel = resolve_kernel(ctx);
+    if (kernel == GG_KERNEL_RESIDENT && ctx->opt_kernel == GG_KERNEL_AUTO && n < kResidentMinSteps)
+        kernel = GG_KERNEL_STREAM2;   // a cooperative launch does not pay for a handful of steps
+    if (kernel == GG_KERNEL_RESIDENT) {
+        int rc = build_plan_resident(ctx);
+        if (rc) return rc;
+        GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+        rc = launch_resident(ctx, ctx->cur, n, dt);
+        if (rc) return rc;
+        ctx->cur ^= 1;
+        ctx->launches += 1;
+        GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+        ctx->timed = true;
+        return GG_OK;
+    }
     if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ||
         kernel == GG_KERNEL_QUAD) {
         int rc = build_plan(ctx, false);
@@ -655,6 +697,11 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
                 value == GG_KERNEL_QUAD) {
                 if (!stream_shape_ok(ctx))
                     return fail(ctx, GG_ERR_UNSUPPORTED, "stream kernel needs nx*sizeof(elem) %% 16 == 0 (nx = %d)", ctx->nx);
+                break;
+            }
+            if (value == GG_KERNEL_RESIDENT) {
+                if (resident_rows(ctx, 148) == 0)
+                    return fail(ctx, GG_ERR_UNSUPPORTED, "resident kernel: %d x %d x %d does not fit on chip", ctx->nx, ctx->ny, ctx->nbatch);
                 break;
             }
             return fail(ctx, GG_ERR_UNSUPPORTED, "gg_set_option: kernel %lld not available", value);

@@ -114,7 +114,7 @@ def test_options_validate():
         binding.gg_destroy(ctx)
     ctx = binding.gg_create(12, 8, 0.5, 1.0, 10.0, 1e-3, 1.0, binding.GG_F32)
     try:
-        assert binding.gg_kernel_used(ctx) == binding.GG_KERNEL_STREAM2  # AUTO: two steps per launch
+        assert binding.gg_kernel_used(ctx) == binding.GG_KERNEL_RESIDENT  # AUTO: tiny grids stay on chip
     finally:
         binding.gg_destroy(ctx)
 

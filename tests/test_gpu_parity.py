@@ -16,15 +16,20 @@ pytestmark = pytest.mark.gpu
 TOL = {"f64": 1e-10, "f32": 2e-4}
 KERNELS = {"generic": binding.GG_KERNEL_GENERIC, "stream": binding.GG_KERNEL_STREAM,
            "stream2": binding.GG_KERNEL_STREAM2, "pair": binding.GG_KERNEL_PAIR,
-           "quad": binding.GG_KERNEL_QUAD}
+           "quad": binding.GG_KERNEL_QUAD, "resident": binding.GG_KERNEL_RESIDENT}
 
 
-def expected_launches(kernel, calls):
-    """Kernel launches for a list of gg_step(n) calls: stream2 advances two steps per launch."""
+def expected_launches(kernel, calls, explicit=True):
+    """Kernel launches for a list of gg_step(n) calls: stream2 / pair advance two steps per launch,
+    quad four (then two, then one), resident all n steps of a call (under AUTO only for calls of
+    at least 8 steps; shorter ones run stream2)."""
+    two = lambda n: n // 2 + n % 2
+    if kernel == "resident":
+        return sum((1 if n > 0 else 0) if (explicit or n >= 8) else two(n) for n in calls)
     if kernel == "quad":
         return sum(n // 4 + (n % 4) // 2 + n % 2 for n in calls)
     if kernel in ("stream2", "pair"):
-        return sum(n // 2 + n % 2 for n in calls)
+        return sum(two(n) for n in calls)
     return sum(calls)
 
 
@@ -46,7 +51,7 @@ def gpu_run(wl, steps, dtype="f64", kernel=None, options=(), split=None):
         used = sim.kernel
         launches = sim.launches
         out = sim.get_state_numpy()
-    assert launches == expected_launches(used, split or [steps])
+    assert launches == expected_launches(used, split or [steps], explicit=kernel is not None)
     return out, used
 
 
@@ -73,7 +78,7 @@ def test_config0_full(kernel):
 def test_config1_full():
     wl = workloads.make(1)
     got, used = gpu_run(wl, wl.steps)
-    assert used == "stream2"   # AUTO: a 512^2 grid is launch-latency bound; two steps per launch
+    assert used == "resident"  # AUTO: a 512^2 grid stays on chip, one cooperative launch per call
     ref = oracle_run(wl, wl.steps)
     assert_close(got, ref, "f64", "cfg1")
 
@@ -342,6 +347,45 @@ def test_quad_configs_long_runs_bit_identical_to_single_step():
     wl = workloads.random_problem(7, 328, 150, batch=2, dy_ratio=0.6)
     got, _ = gpu_run(wl, 32, kernel="quad")
     assert_close(got, oracle_run(wl, 32), "f64", "quad dx != dy")
+
+
+# ---------------------------------------------------------------------------------------------
+# GG_KERNEL_RESIDENT: all n steps in one cooperative launch, state in shared memory
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_resident_shapes_batches_and_ragged_slabs(dtype):
+    for nx, ny, batch in ((4, 2, 1), (8, 3, 2), (60, 17, 3), (64, 64, 1), (124, 41, 3), (200, 297, 1),
+                          (512, 150, 1), (328, 150, 2)):
+        if dtype == "f64" and nx > 512:
+            continue
+        wl = workloads.random_problem(500 + nx, nx, ny, batch=batch)
+        for n in (1, 2, 9):
+            got, used = gpu_run(wl, n, dtype=dtype, kernel="resident")
+            assert used == "resident"
+            assert_close(got, oracle_run(wl, n), dtype, f"resident {dtype} {nx}x{ny}x{batch} n={n}")
+
+
+def test_resident_long_runs_bit_identical_to_single_step():
+    for wl, n in ((workloads.make(0), 200), (workloads.make(1, nx=256, ny=512, steps=400), 401),
+                  (workloads.make(4, nx=264, ny=90, batch=5, steps=60), 60),
+                  (workloads.random_problem(8, 328, 150, batch=2, dy_ratio=0.6), 33)):
+        a, _ = gpu_run(wl, n, kernel="resident", split=[1, 2, 0, 7, n - 10])
+        b, _ = gpu_run(wl, n, kernel="stream")
+        for x, y in zip(a, b):
+            assert np.array_equal(x, y)
+        assert_close(a, oracle_run(wl, n), "f64", f"resident {wl.name}")
+
+
+def test_resident_refuses_grids_that_do_not_fit():
+    wl = workloads.make(2, nx=1024, ny=64, steps=1)          # 8 KB rows: more than 256 lanes
+    with binding.from_workload(wl) as sim:
+        assert sim.kernel != "resident"
+        with pytest.raises(binding.GGError) as e:
+            sim.set_option(binding.GG_OPT_KERNEL, binding.GG_KERNEL_RESIDENT)
+        assert e.value.code == binding.GG_ERR_UNSUPPORTED
+    wl = workloads.make(2, nx=64, ny=4096, steps=1)          # 4096 rows: more slabs than SMs
+    with binding.from_workload(wl) as sim:
+        assert sim.kernel != "resident"
 
 
 def test_split_calls_equal_one_call():
