@@ -165,11 +165,16 @@ int resolve_kernel(const gg_ctx* c) {
     // Tuned on B200.  The deeper the temporal blocking, the larger the
     // per-launch pipeline fill and the halo overhead, so small grids stay with shallower kernels.
     const double cells = (double)c->nx * c->ny * c->nbatch;
-    // grids that fit on chip: one cooperative launch for the whole call (gg_step uses it for
-    // calls of at least kResidentMinSteps steps and STREAM2 for shorter ones)
-    if (resident_rows(c, c->bound ? (c->num_sms < 148 ? c->num_sms : 148) : 148) > 0) return GG_KERNEL_RESIDENT;
+    // Small grids are launch-latency bound.  Grids that fit on chip run the
+    // whole call in one cooperative launch where that measured faster: fp32 up to 512^2, fp64 up
+    // to 128^2 (gg_step uses it for calls of >= kResidentMinSteps steps, STREAM2 for shorter ones).
+    if ((c->dtype == GG_F32 || cells <= 16384.0) &&
+        resident_rows(c, c->bound ? (c->num_sms < 148 ? c->num_sms : 148) : 148) > 0)
+        return GG_KERNEL_RESIDENT;
     if (c->dtype == GG_F64 && c->nx >= 4096 && cells >= 16777216.0) return GG_KERNEL_QUAD;
     if (cells > 262144.0 && c->nx >= 240) return GG_KERNEL_PAIR;
+    // mid-size fp64 grids: four steps per launch cost a flat ~4.9 us per step
+    if (c->dtype == GG_F64 && c->nx >= 236 && cells >= 65536.0) return GG_KERNEL_QUAD;
     return GG_KERNEL_STREAM2;
 }
 

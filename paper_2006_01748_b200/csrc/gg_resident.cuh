@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_resident(const ResidentArgs A)
         if (last) break;
         __syncthreads();   // the pong copy and this step's edge rows are written
         if (t == 0) {
-            __threadfence();
+            __threadfence();   // (measured: faster than leaving the whole flush to the release)
             st_release_gpu(A.flags + slab, A.epoch + (unsigned int)step);
         }
         // wait for the neighbours' edge rows of this step (same simulation only)

@@ -78,7 +78,7 @@ def test_config0_full(kernel):
 def test_config1_full():
     wl = workloads.make(1)
     got, used = gpu_run(wl, wl.steps)
-    assert used == "resident"  # AUTO: a 512^2 grid stays on chip, one cooperative launch per call
+    assert used == "quad"      # AUTO: mid-size fp64 grids run four steps per launch
     ref = oracle_run(wl, wl.steps)
     assert_close(got, ref, "f64", "cfg1")
 
@@ -383,7 +383,7 @@ def test_resident_refuses_grids_that_do_not_fit():
         with pytest.raises(binding.GGError) as e:
             sim.set_option(binding.GG_OPT_KERNEL, binding.GG_KERNEL_RESIDENT)
         assert e.value.code == binding.GG_ERR_UNSUPPORTED
-    wl = workloads.make(2, nx=64, ny=4096, steps=1)          # 4096 rows: more slabs than SMs
+    wl = workloads.make(2, nx=64, ny=16384, steps=1)         # more 64-row slabs than SMs
     with binding.from_workload(wl) as sim:
         assert sim.kernel != "resident"
 
