@@ -110,3 +110,24 @@ def test_config4_full_size_batch_sampled():
         check_windows(wl, s, got, n, spots, "f64")
     # simulations with different d must have diverged from one another
     assert np.max(np.abs(got[0][0] - got[0][62])) > 1e-6
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_large_ragged_grid_sampled(dtype):
+    """A grid wider than the headline one in cells per row for fp32 tiles, ragged against every
+    tile width of the library (236 / 480 / 944 / 1888 cells) and against the row chunks: 10008 x
+    5001 cells, AUTO kernel, six steps (fp64: one four-step + one two-step launch)."""
+    wl = workloads.make(3, nx=10008, ny=5001)
+    n = 6
+    with binding.from_workload(wl, dtype=dtype) as sim:
+        assert sim.kernel == ("quad" if dtype == "f64" else "pair")
+        sim.step(n, wl.dt)
+        got = sim.get_state_numpy()
+    for g in got:
+        assert np.isfinite(g).all()
+    nx, ny = wl.nx, wl.ny
+    spots = [(0, 0), (nx - WIN, 0), (0, ny - WIN), (nx - WIN, ny - WIN),
+             (nx - 24, 0, 24, ny),            # the ragged last tile column, every row chunk
+             (0, ny - 24, nx, 24),            # the top rows, every tile column
+             (9912 - 12, 2500, 24, 200)]      # 42 x 236: the last full four-step tile seam
+    check_windows(wl, 0, got, n, spots, dtype)
