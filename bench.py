@@ -258,9 +258,30 @@ def run_ours(args, wl, rank, world, device):
            "seconds": e2e_s}
     final = tuple(out[k].numpy() for k in ("U", "V", "W"))
     kernel = sim.kernel
+    reductions = None
+    if args.extras:
+        # the device-side reductions next to the step: one pass over
+        # U, V, W resp. a, b, c = 3 arrays read; wall clock around the synchronising C-ABI call
+        # (includes the launch and the 8..64-byte result copy), median of 7
+        es = 8 if dtype == "f64" else 4
+
+        def timed(fn):
+            ts = []
+            for _ in range(7):
+                torch.cuda.synchronize(device)
+                t0 = time.perf_counter()
+                fn()
+                ts.append(time.perf_counter() - t0)
+            return float(np.median(ts))
+        t_diag = timed(lambda: sim.diagnostics(1e-2))
+        t_dt = timed(lambda: sim.max_stable_dt(0.2))
+        reductions = {"gg_diagnostics_ms": t_diag * 1e3, "gg_diagnostics_gbs": 3 * cells * es / t_diag / 1e9,
+                      "gg_max_stable_dt_ms": t_dt * 1e3,
+                      "gg_max_stable_dt_gbs": 3 * wl.nx * wl.ny * es / t_dt / 1e9,
+                      "bound": "hbm", "bytes": "3 arrays read once, 24 B (fp64) / 12 B (fp32) per cell"}
     sim.close()
     return dict(value=value, ms=ms / K, reps_ms=reps, launches=launches, e2e=e2e,
-                clocks=clk.summary(), kernel=kernel, final=final)
+                clocks=clk.summary(), kernel=kernel, final=final, reductions=reductions)
 
 
 def sampled_parity(wl, final, K, size=48):
@@ -303,6 +324,8 @@ def main():
     ap.add_argument("--reps", type=int, default=3)
     ap.add_argument("--n", type=int, default=8192, help="grid edge (8192 = the headline config)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--extras", action="store_true",
+                    help="also time gg_diagnostics / gg_max_stable_dt (adds a `reductions` object)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -376,6 +399,8 @@ def main():
             line["alu"] = {"bound": "alu", "achieved": alu, "peak": alu_peak,
                            "unit": f"T {args.dtype} instr/s", "frac": alu / alu_peak,
                            "instr_per_cell_step": ops}
+        if res.get("reductions"):
+            line["reductions"] = res["reductions"]
         t0 = time.perf_counter()
         line["parity_sample_max_abs_err"] = sampled_parity(wl, res["final"], args.steps)
         log(f"sampled parity: {line['parity_sample_max_abs_err']:.3e} ({time.perf_counter() - t0:.1f} s)")

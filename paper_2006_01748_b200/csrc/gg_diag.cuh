@@ -76,8 +76,30 @@ gg_diag_partial(const T* __restrict__ U, const T* __restrict__ V, const T* __res
     const size_t hi = lo + seg < plane ? lo + seg : plane;
     DiagAcc acc;
     acc.init();
-    for (size_t q = lo + threadIdx.x; q < hi; q += kDiagThreads)
-        acc.cell((double)U[base + q], (double)V[base + q], (double)W[base + q], eps);
+    constexpr int VC = 16 / (int)sizeof(T);           // cells per 16-byte vector
+    constexpr int UN = 4;                             // vectors in flight per thread and array
+    const T* pu = U + base; const T* pv = V + base; const T* pw = W + base;
+    size_t q = lo;
+    if ((plane * sizeof(T)) % 16 == 0 && lo % VC == 0) {
+        // 16-byte loads, UN x 3 of them in flight per thread (the pass is HBM-bound)
+        const size_t stride = (size_t)kDiagThreads * VC * UN;
+        for (; q + stride <= hi; q += stride) {
+            T u[UN][VC], v[UN][VC], w[UN][VC];
+#pragma unroll
+            for (int n = 0; n < UN; ++n) {
+                const size_t e = q + ((size_t)n * kDiagThreads + threadIdx.x) * VC;
+                *reinterpret_cast<uint4*>(u[n]) = *reinterpret_cast<const uint4*>(pu + e);
+                *reinterpret_cast<uint4*>(v[n]) = *reinterpret_cast<const uint4*>(pv + e);
+                *reinterpret_cast<uint4*>(w[n]) = *reinterpret_cast<const uint4*>(pw + e);
+            }
+#pragma unroll
+            for (int n = 0; n < UN; ++n)
+#pragma unroll
+                for (int c = 0; c < VC; ++c) acc.cell((double)u[n][c], (double)v[n][c], (double)w[n][c], eps);
+        }
+    }
+    for (q += threadIdx.x; q < hi; q += kDiagThreads)   // tail (or unaligned planes): scalar
+        acc.cell((double)pu[q], (double)pv[q], (double)pw[q], eps);
     diag_block_reduce(acc, sh);
     if (threadIdx.x == 0) {
         double* o = partial + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * kDiagCount;
@@ -110,11 +132,31 @@ gg_lambda_max_partial(const T* __restrict__ a, const T* __restrict__ b, const T*
     const size_t lo = (size_t)blockIdx.x * seg;
     const size_t hi = lo + seg < plane ? lo + seg : plane;
     double m = -INFINITY;
-    for (size_t q = lo + threadIdx.x; q < hi; q += kDiagThreads) {
-        const double aa = (double)a[q], bb = (double)b[q], cc = (double)c[q];
+    auto lam = [](double aa, double bb, double cc) {
         const double hd = 0.5 * (aa - cc);
-        m = fmax(m, 0.5 * (aa + cc) + sqrt(hd * hd + bb * bb));
+        return 0.5 * (aa + cc) + sqrt(hd * hd + bb * bb);
+    };
+    constexpr int VC = 16 / (int)sizeof(T);
+    constexpr int UN = 4;
+    size_t q = lo;
+    if ((plane * sizeof(T)) % 16 == 0 && lo % VC == 0) {
+        const size_t stride = (size_t)kDiagThreads * VC * UN;
+        for (; q + stride <= hi; q += stride) {
+            T va[UN][VC], vb[UN][VC], vc[UN][VC];
+#pragma unroll
+            for (int n = 0; n < UN; ++n) {
+                const size_t e = q + ((size_t)n * kDiagThreads + threadIdx.x) * VC;
+                *reinterpret_cast<uint4*>(va[n]) = *reinterpret_cast<const uint4*>(a + e);
+                *reinterpret_cast<uint4*>(vb[n]) = *reinterpret_cast<const uint4*>(b + e);
+                *reinterpret_cast<uint4*>(vc[n]) = *reinterpret_cast<const uint4*>(c + e);
+            }
+#pragma unroll
+            for (int n = 0; n < UN; ++n)
+#pragma unroll
+                for (int k = 0; k < VC; ++k) m = fmax(m, lam((double)va[n][k], (double)vb[n][k], (double)vc[n][k]));
+        }
     }
+    for (q += threadIdx.x; q < hi; q += kDiagThreads) m = fmax(m, lam((double)a[q], (double)b[q], (double)c[q]));
     sh[threadIdx.x] = m;
     __syncthreads();
     for (int s = kDiagThreads / 2; s > 0; s >>= 1) {
