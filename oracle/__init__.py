@@ -98,6 +98,7 @@ def step(U, V, W, a, b, c, *, r: float, d: float, alpha: float, c_r: float, n: i
 # ---------------------------------------------------------------------------------------------
 # Reductions next to the step.  Plain NumPy, written out.
 # Pins: tests/test_oracle_pins.py (brute-force loops on tiny grids, eigvalsh, closed forms).
+# "parity unpinned": the step-size RULE of max_stable_dt (reading A6; the paper prints none).
 # ---------------------------------------------------------------------------------------------
 DIAG_NAMES = ("sum_U", "sum_V", "sum_W", "gap_cells", "tumour_cells", "min_W", "max_U", "max_W")
 
@@ -124,7 +125,11 @@ def lambda_max(a, b, c) -> float:
 
 def max_stable_dt(a, b, c, alpha, dx: float, dy: float | None = None, safety: float = 0.2) -> float:
     """DESIGN.md reading A6 (the paper prints no formula):
-    safety * min(dx,dy)^2 / max(max alpha, lambda_max(A))."""
+    safety * min(dx,dy)^2 / max(max alpha, lambda_max(A)).
+
+    PARITY UNPINNED as far as the RULE goes: the paper says only that the host recomputes the step
+    "to ensure numerical stability"; nothing it prints fixes this formula (lambda_max itself is
+    pinned against LAPACK and closed forms, and the arithmetic of the rule against worked values)."""
     if dy is None:
         dy = dx
     rate = max(float(np.max(alpha)), lambda_max(a, b, c))

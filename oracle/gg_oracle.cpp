@@ -24,7 +24,8 @@
 // one full step (tests/golden/*.txt), polynomial / plane-wave closed forms, uniform data -> ODE
 // recursion, equilibria, conservation of sum W and sum V, 1-D reduction against an independent
 // 1-D code, transpose / flip / rotation symmetries, discrete cosine eigenmodes over many steps,
-// bounds for b = 0.  Nothing on this path is "parity unpinned".
+// bounds for b = 0.  Nothing on this path is "parity unpinned".  (The NumPy reductions in
+// oracle/__init__.py carry one unpinned item: the step-size RULE of max_stable_dt, reading A6.)
 //
 // Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).  OpenMP only
 // splits rows; every output cell depends on time-k data only, so the result is bit-identical for
