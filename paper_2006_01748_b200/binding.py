@@ -267,12 +267,14 @@ class Simulation:
     def set_tensor(self, a, b, c):
         sh = (self.ny, self.nx)
         ta, tb, tc = (self._dev(x, sh) for x in (a, b, c))
+        self._after_current_stream()
         gg_set_tensor(self.ctx, ta.data_ptr(), tb.data_ptr(), tc.data_ptr())
         self._sync()  # temporaries may be freed after return
 
     def set_state(self, U, V, W):
         sh = (self.batch, self.ny, self.nx)
         tU, tV, tW = (self._dev(x, sh) for x in (U, V, W))
+        self._after_current_stream()
         gg_set_state(self.ctx, tU.data_ptr(), tV.data_ptr(), tW.data_ptr())
         self._sync()
 
@@ -324,6 +326,12 @@ class Simulation:
 
     def last_step_ms(self) -> float:
         return gg_last_step_ms(self.ctx)
+
+    def _after_current_stream(self):
+        """libgg enqueues on the bound stream; tensors staged by torch live on torch's current
+        stream: order the bound stream after it (stream plumbing only)."""
+        if self.stream is not None:
+            self.stream.wait_stream(self.torch.cuda.current_stream(self.device))
 
     def _sync(self):
         if self.stream is None:

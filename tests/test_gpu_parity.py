@@ -388,6 +388,25 @@ def test_resident_refuses_grids_that_do_not_fit():
         assert sim.kernel != "resident"
 
 
+def test_user_stream_every_auto_path():
+    """The library enqueues on the stream given to gg_bind: run the resident, quad, pair and
+    generic paths on a non-default stream while the default stream is kept busy."""
+    import torch
+    stream = torch.cuda.Stream()
+    busy = torch.empty(64 << 20, device="cuda")
+    for wl, n, want in ((workloads.make(0), 40, "resident"),
+                        (workloads.make(1, nx=512, ny=160, steps=1), 24, "quad"),
+                        (workloads.make(4, nx=264, ny=1100, batch=2, steps=1), 10, "pair"),
+                        (workloads.random_problem(3, 41, 23), 9, "generic")):
+        for _ in range(4):
+            busy.add_(1.0)                       # unrelated work on the default stream
+        with binding.from_workload(wl, stream=stream) as sim:
+            assert sim.kernel == want
+            sim.step(n, wl.dt)
+            got = sim.get_state_numpy()
+        assert_close(got, oracle_run(wl, n), "f64", f"user stream {want}")
+
+
 def test_split_calls_equal_one_call():
     wl = workloads.make(1, nx=128, ny=96)
     a, _ = gpu_run(wl, 37)
