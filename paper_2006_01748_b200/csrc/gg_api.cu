@@ -171,10 +171,11 @@ int resolve_kernel(const gg_ctx* c) {
     if ((c->dtype == GG_F32 || cells <= 16384.0) &&
         resident_rows(c, c->bound ? (c->num_sms < 148 ? c->num_sms : 148) : 148) > 0)
         return GG_KERNEL_RESIDENT;
-    if (c->dtype == GG_F64 && c->nx >= 4096 && cells >= 16777216.0) return GG_KERNEL_QUAD;
-    if (cells > 262144.0 && c->nx >= 240) return GG_KERNEL_PAIR;
-    // mid-size fp64 grids: four steps per launch cost a flat ~4.9 us per step
+    // fp64 from mid-size grids up: four steps per launch (measured ahead of the pair kernel from
+    // 512^2 to 8192^2 and on batches; a flat ~4.9 us per step below that)
     if (c->dtype == GG_F64 && c->nx >= 236 && cells >= 65536.0) return GG_KERNEL_QUAD;
+    // fp32 (issue-bound with 4 cells per lane): two steps per launch in registers
+    if (cells > 262144.0 && c->nx >= 240) return GG_KERNEL_PAIR;
     return GG_KERNEL_STREAM2;
 }
 

@@ -394,17 +394,17 @@ def test_user_stream_every_auto_path():
     import torch
     stream = torch.cuda.Stream()
     busy = torch.empty(64 << 20, device="cuda")
-    for wl, n, want in ((workloads.make(0), 40, "resident"),
-                        (workloads.make(1, nx=512, ny=160, steps=1), 24, "quad"),
-                        (workloads.make(4, nx=264, ny=1100, batch=2, steps=1), 10, "pair"),
-                        (workloads.random_problem(3, 41, 23), 9, "generic")):
+    for wl, n, want, dtype in ((workloads.make(0), 40, "resident", "f64"),
+                               (workloads.make(1, nx=512, ny=160, steps=1), 24, "quad", "f64"),
+                               (workloads.make(3, nx=2048, ny=160, steps=1), 10, "pair", "f32"),
+                               (workloads.random_problem(3, 41, 23), 9, "generic", "f64")):
         for _ in range(4):
             busy.add_(1.0)                       # unrelated work on the default stream
-        with binding.from_workload(wl, stream=stream) as sim:
+        with binding.from_workload(wl, dtype=dtype, stream=stream) as sim:
             assert sim.kernel == want
             sim.step(n, wl.dt)
             got = sim.get_state_numpy()
-        assert_close(got, oracle_run(wl, n), "f64", f"user stream {want}")
+        assert_close(got, oracle_run(wl, n), dtype, f"user stream {want}")
 
 
 def test_split_calls_equal_one_call():
