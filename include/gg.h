@@ -158,6 +158,14 @@ enum {
 };
 int gg_diagnostics(gg_ctx* ctx, double eps, double* out);
 
+/* Front position along a grid line (the paper reads the tumour and acid fronts and the gap between
+ * them off the fields): for every simulation the first and the last cell index
+ * along row `index` (axis 0: the line runs along x) or column `index` (axis 1: along y) where
+ * field `field` (0 = U, 1 = V, 2 = W) is >= level; (-1, -1) if no cell qualifies.  out: HOST array
+ * [nbatch][2] of int.  The comparison is made on the stored values converted exactly to double.
+ * Synchronises the bound stream. */
+int gg_front(gg_ctx* ctx, int field, int axis, int index, double level, int* out);
+
 /* Step-size bound for the explicit scheme (PAPER.md:62, :79, :128 say the host recomputes dt "to
  * ensure numerical stability" and print no formula; reading A6 is used):
  *     *dt = safety * min(dx,dy)^2 / max(max_s alpha_s, lambda_max),

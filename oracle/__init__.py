@@ -134,3 +134,13 @@ def max_stable_dt(a, b, c, alpha, dx: float, dy: float | None = None, safety: fl
         dy = dx
     rate = max(float(np.max(alpha)), lambda_max(a, b, c))
     return safety * min(dx, dy) ** 2 / rate
+
+
+def front(F, axis: int, index: int, level: float):
+    """First and last cell index along row `index` (axis 0: the line runs along x) or column
+    `index` (axis 1) of one field [ny][nx] where the field is >= level; (-1, -1) if none.  The
+    positions of the tumour and acid fronts along a ray."""
+    F = _c(F)
+    line = F[index, :] if axis == 0 else F[:, index]
+    idx = np.nonzero(line >= level)[0]
+    return (int(idx[0]), int(idx[-1])) if idx.size else (-1, -1)

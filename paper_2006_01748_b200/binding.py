@@ -53,6 +53,8 @@ SIGNATURES = {
     "gg_get_state_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_diagnostics": (ctypes.c_int, [_vp, ctypes.c_double, _dp]),
     "gg_max_stable_dt": (ctypes.c_int, [_vp, ctypes.c_double, _dp, _dp]),
+    "gg_front": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                ctypes.POINTER(ctypes.c_int)]),
     "gg_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_longlong]),
     "gg_kernel_used": (ctypes.c_int, [_vp]),
     "gg_launches": (ctypes.c_longlong, [_vp]),
@@ -168,6 +170,14 @@ def gg_diagnostics(ctx, eps: float, nbatch: int) -> np.ndarray:
     """[nbatch][GG_DIAG_COUNT] doubles, slot order GG_DIAG_NAMES."""
     out = np.empty((nbatch, GG_DIAG_COUNT), dtype=np.float64)
     _check(ctx, load().gg_diagnostics(ctx, float(eps), out.ctypes.data_as(_dp)))
+    return out
+
+
+def gg_front(ctx, field: int, axis: int, index: int, level: float, nbatch: int) -> np.ndarray:
+    """[nbatch][2] ints: first and last cell index along the line with field >= level, or -1."""
+    out = np.empty((nbatch, 2), dtype=np.int32)
+    _check(ctx, load().gg_front(ctx, int(field), int(axis), int(index), float(level),
+                                out.ctypes.data_as(ctypes.POINTER(ctypes.c_int))))
     return out
 
 
@@ -308,6 +318,9 @@ class Simulation:
 
     def diagnostics(self, eps=1e-2):
         return gg_diagnostics(self.ctx, eps, self.batch)
+
+    def front(self, field, axis, index, level=0.5):
+        return gg_front(self.ctx, {"U": 0, "V": 1, "W": 2}.get(field, field), axis, index, level, self.batch)
 
     def max_stable_dt(self, safety=0.2):
         return gg_max_stable_dt(self.ctx, safety)

@@ -783,6 +783,31 @@ int gg_diagnostics(gg_ctx* ctx, double eps, double* out) {
     return GG_OK;
 }
 
+int gg_front(gg_ctx* ctx, int field, int axis, int index, double level, int* out) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound || !ctx->have_state) return fail(ctx, GG_ERR_STATE, "gg_front: no state set");
+    if (!out) return fail(ctx, GG_ERR_ARG, "gg_front: out is NULL");
+    if (field < 0 || field > 2) return fail(ctx, GG_ERR_ARG, "gg_front: field must be 0 (U), 1 (V) or 2 (W)");
+    if (axis != 0 && axis != 1) return fail(ctx, GG_ERR_ARG, "gg_front: axis must be 0 (along x) or 1 (along y)");
+    const int len = axis == 0 ? ctx->nx : ctx->ny, other = axis == 0 ? ctx->ny : ctx->nx;
+    if (index < 0 || index >= other) return fail(ctx, GG_ERR_ARG, "gg_front: line index %d outside [0, %d)", index, other);
+    if (!std::isfinite(level)) return fail(ctx, GG_ERR_ARG, "gg_front: level must be finite");
+    if ((size_t)ctx->nbatch * 2 * sizeof(int) > scratch_doubles(ctx) * sizeof(double))
+        return fail(ctx, GG_ERR_UNSUPPORTED, "gg_front: scratch too small");
+    const size_t offset = axis == 0 ? (size_t)index * ctx->nx : (size_t)index;
+    const size_t stride = axis == 0 ? 1 : (size_t)ctx->nx;
+    int* d_out = (int*)ctx->d_scratch;
+    const void* F = ctx->state[ctx->cur][field];
+    if (ctx->dtype == GG_F64)
+        gg::gg_front_line<double><<<ctx->nbatch, gg::kDiagThreads, 0, ctx->stream>>>((const double*)F, ctx->plane(), offset, stride, len, level, d_out);
+    else
+        gg::gg_front_line<float><<<ctx->nbatch, gg::kDiagThreads, 0, ctx->stream>>>((const float*)F, ctx->plane(), offset, stride, len, level, d_out);
+    GG_CUDA(ctx, cudaGetLastError());
+    GG_CUDA(ctx, cudaMemcpyAsync(out, d_out, (size_t)ctx->nbatch * 2 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return GG_OK;
+}
+
 int gg_max_stable_dt(gg_ctx* ctx, double safety, double* dt, double* lambda_max) {
     if (!ctx) return GG_ERR_ARG;
     if (!ctx->bound || !ctx->have_tensor) return fail(ctx, GG_ERR_STATE, "gg_max_stable_dt: no tensor set");

@@ -166,4 +166,32 @@ gg_lambda_max_partial(const T* __restrict__ a, const T* __restrict__ b, const T*
     if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
 }
 
+// Front position along a grid line ("front position along a ray"): the first
+// and the last cell index q in [0, len) with F[q*stride] >= level along one row (stride 1) or one
+// column (stride nx) of field F of every simulation; (-1, -1) if no cell qualifies.  One block
+// per simulation; min / max over the qualifying indices, so the result is order-independent.
+template <typename T>
+__global__ void __launch_bounds__(kDiagThreads)
+gg_front_line(const T* __restrict__ F, size_t plane, size_t offset, size_t stride, int len,
+              double level, int* __restrict__ out) {
+    __shared__ int lo[kDiagThreads], hi[kDiagThreads];
+    const T* p = F + (size_t)blockIdx.x * plane + offset;
+    int a = len, b = -1;
+    for (int q = threadIdx.x; q < len; q += kDiagThreads)
+        if ((double)p[(size_t)q * stride] >= level) { a = min(a, q); b = max(b, q); }
+    lo[threadIdx.x] = a; hi[threadIdx.x] = b;
+    __syncthreads();
+    for (int s = kDiagThreads / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) {
+            lo[threadIdx.x] = min(lo[threadIdx.x], lo[threadIdx.x + s]);
+            hi[threadIdx.x] = max(hi[threadIdx.x], hi[threadIdx.x + s]);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        out[2 * blockIdx.x + 0] = hi[0] < 0 ? -1 : lo[0];
+        out[2 * blockIdx.x + 1] = hi[0];
+    }
+}
+
 }  // namespace gg

@@ -117,3 +117,22 @@ def test_reduction_call_order_errors():
             assert e.value.code == binding.GG_ERR_ARG
         with pytest.raises(binding.GGError):
             sim.max_stable_dt(0.0)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_front_positions(dtype):
+    wl = workloads.make(4, nx=264, ny=190, batch=4, steps=200)
+    with binding.from_workload(wl, dtype=dtype) as sim:
+        sim.step(wl.steps, wl.dt)
+        U, V, W = sim.get_state_numpy()
+        fields = {"U": U, "V": V, "W": W}
+        for field, level in (("V", 0.5), ("W", 0.2), ("U", 0.9), ("V", 2.0)):
+            for axis, index in ((0, 0), (0, 114), (0, 189), (1, 0), (1, 92), (1, 263)):
+                got = sim.front(field, axis, index, level)
+                for s in range(wl.batch):
+                    assert tuple(got[s]) == oracle.front(fields[field][s], axis, index, level)
+        with pytest.raises(binding.GGError) as e:
+            sim.front("V", 0, 190, 0.5)
+        assert e.value.code == binding.GG_ERR_ARG
+        with pytest.raises(binding.GGError):
+            sim.front(3, 0, 0, 0.5)

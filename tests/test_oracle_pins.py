@@ -496,3 +496,21 @@ def test_gap_opens_for_large_d_only():
                               dt=wl.dt, dx=wl.h)
         gaps[d] = oracle.diagnostics(U, V, W, 0.2)[3]
     assert gaps[0.5] == 0 and gaps[40.0] > 100
+
+
+def test_front_positions_brute_force_and_disk():
+    rng = np.random.default_rng(7)
+    F = rng.uniform(0, 1, (6, 9))
+    for axis, n in ((0, 6), (1, 9)):
+        for index in range(n):
+            line = [F[index][i] for i in range(9)] if axis == 0 else [F[j][index] for j in range(6)]
+            hits = [q for q, x in enumerate(line) if x >= 0.6]
+            want = (hits[0], hits[-1]) if hits else (-1, -1)
+            assert oracle.front(F, axis, index, 0.6) == want
+    assert oracle.front(np.zeros((4, 5)), 0, 2, 0.5) == (-1, -1)
+    assert oracle.front(np.full((4, 5), 0.5), 1, 3, 0.5) == (0, 3)      # >= is inclusive
+    # the seeded disk of config 0 (radius 6.4 cells about the centre of a 64^2 grid): along the
+    # centre row the tumour occupies the cells whose centres lie within the disk
+    wl = workloads.make(0)
+    lo, hi = oracle.front(wl.V[0], 0, 32, 0.5)
+    assert (lo, hi) == (26, 37) and oracle.front(wl.V[0], 1, 32, 0.5) == (26, 37)
