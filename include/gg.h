@@ -154,7 +154,8 @@ enum {
     GG_DIAG_MIN_W = 5,   /* min W (negative: undershoot, reading A7)   */
     GG_DIAG_MAX_U = 6,   /* max U (> 1: overshoot)                     */
     GG_DIAG_MAX_W = 7,   /* max W                                      */
-    GG_DIAG_COUNT = 8
+    GG_DIAG_NONFINITE = 8, /* #{(i,j): U, V or W is NaN or +-Inf} (min/max skip NaNs) */
+    GG_DIAG_COUNT = 9
 };
 int gg_diagnostics(gg_ctx* ctx, double eps, double* out);
 

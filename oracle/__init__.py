@@ -100,20 +100,25 @@ def step(U, V, W, a, b, c, *, r: float, d: float, alpha: float, c_r: float, n: i
 # Pins: tests/test_oracle_pins.py (brute-force loops on tiny grids, eigvalsh, closed forms).
 # "parity unpinned": the step-size RULE of max_stable_dt (reading A6; the paper prints none).
 # ---------------------------------------------------------------------------------------------
-DIAG_NAMES = ("sum_U", "sum_V", "sum_W", "gap_cells", "tumour_cells", "min_W", "max_U", "max_W")
+DIAG_NAMES = ("sum_U", "sum_V", "sum_W", "gap_cells", "tumour_cells", "min_W", "max_U", "max_W",
+              "nonfinite_cells")
 
 
 def diagnostics(U, V, W, eps: float) -> np.ndarray:
     """Diagnostics of one state [ny][nx], in the order DIAG_NAMES: the sums of the three fields,
     the number of interstitial-gap cells (U < eps and V < eps: neither cell type present, the gap
     between the fronts of PAPER.md:100-111), the number of tumour cells (V >= 1/2), min W, max U,
-    max W.  Everything in fp64."""
+    max W (NaNs skipped, as fmin / fmax do), and the number of cells where U, V or W is not finite.
+    Everything in fp64."""
     U, V, W = _c(U), _c(V), _c(W)
     return np.array([
         np.sum(U), np.sum(V), np.sum(W),
         float(np.count_nonzero((U < eps) & (V < eps))),
         float(np.count_nonzero(V >= 0.5)),
-        np.min(W), np.max(U), np.max(W)], dtype=np.float64)
+        np.nanmin(W) if np.isfinite(W).any() or np.isinf(W).any() else np.inf,
+        np.nanmax(U) if not np.isnan(U).all() else -np.inf,
+        np.nanmax(W) if not np.isnan(W).all() else -np.inf,
+        float(np.count_nonzero(~(np.isfinite(U) & np.isfinite(V) & np.isfinite(W))))], dtype=np.float64)
 
 
 def lambda_max(a, b, c) -> float:

@@ -162,7 +162,8 @@ def gg_get_state_host(ctx, U_ptr, V_ptr, W_ptr):
     _check(ctx, load().gg_get_state_host(ctx, U_ptr, V_ptr, W_ptr))
 
 
-GG_DIAG_NAMES = ("sum_U", "sum_V", "sum_W", "gap_cells", "tumour_cells", "min_W", "max_U", "max_W")
+GG_DIAG_NAMES = ("sum_U", "sum_V", "sum_W", "gap_cells", "tumour_cells", "min_W", "max_U", "max_W",
+                 "nonfinite_cells")
 GG_DIAG_COUNT = len(GG_DIAG_NAMES)
 
 

@@ -3,8 +3,9 @@
 //  * gg_diag_partial / gg_diag_final: per-simulation diagnostics of the current state without a
 //    full gg_get_state -- the quantities the paper's experiments read off the fields (tumour and
 //    acid mass, the interstitial gap U ~ 0 and V ~ 0 between the fronts): sums of
-//    U, V, W, the gap and tumour cell counts, and the extrema that show the scheme's documented
-//    over/undershoots (reading A7).
+//    U, V, W, the gap and tumour cell counts, the extrema that show the scheme's documented
+//    over/undershoots (reading A7), and the number of cells holding a NaN or Inf (the
+//    step itself never repairs or hides one: eq. (3) has no such rule).
 //  * gg_lambda_max_partial: max over cells of the larger eigenvalue of [[a,b],[b,c]] (eq. (2),
 //    PAPER.md:40), the quantity the explicit step bound needs (DESIGN.md
 //    reading A6).
@@ -18,17 +19,17 @@
 
 namespace gg {
 
-constexpr int kDiagCount = 8;      // == GG_DIAG_COUNT in include/gg.h
+constexpr int kDiagCount = 9;      // == GG_DIAG_COUNT in include/gg.h
 constexpr int kDiagThreads = 256;
 constexpr int kDiagMaxBlocks = 296;  // partial blocks per simulation (2 per SM on B200)
 
 // slot order == GG_DIAG_* in include/gg.h
-enum { kSumU = 0, kSumV, kSumW, kGap, kTumour, kMinW, kMaxU, kMaxW };
+enum { kSumU = 0, kSumV, kSumW, kGap, kTumour, kMinW, kMaxU, kMaxW, kNonFinite };
 
 struct DiagAcc {
     double v[kDiagCount];
     __device__ __forceinline__ void init() {
-        v[kSumU] = v[kSumV] = v[kSumW] = v[kGap] = v[kTumour] = 0.0;
+        v[kSumU] = v[kSumV] = v[kSumW] = v[kGap] = v[kTumour] = v[kNonFinite] = 0.0;
         v[kMinW] = INFINITY;
         v[kMaxU] = v[kMaxW] = -INFINITY;
     }
@@ -39,10 +40,11 @@ struct DiagAcc {
         v[kMinW] = fmin(v[kMinW], w);
         v[kMaxU] = fmax(v[kMaxU], u);
         v[kMaxW] = fmax(v[kMaxW], w);
+        v[kNonFinite] += (isfinite(u) && isfinite(vv) && isfinite(w)) ? 0.0 : 1.0;
     }
     __device__ __forceinline__ void merge(const double* o) {
         v[kSumU] += o[kSumU]; v[kSumV] += o[kSumV]; v[kSumW] += o[kSumW];
-        v[kGap] += o[kGap]; v[kTumour] += o[kTumour];
+        v[kGap] += o[kGap]; v[kTumour] += o[kTumour]; v[kNonFinite] += o[kNonFinite];
         v[kMinW] = fmin(v[kMinW], o[kMinW]);
         v[kMaxU] = fmax(v[kMaxU], o[kMaxU]);
         v[kMaxW] = fmax(v[kMaxW], o[kMaxW]);

@@ -136,3 +136,24 @@ def test_front_positions(dtype):
         assert e.value.code == binding.GG_ERR_ARG
         with pytest.raises(binding.GGError):
             sim.front(3, 0, 0, 0.5)
+
+
+def test_diagnostics_count_nonfinite_cells():
+    """Nothing in the step repairs a NaN (eq. (3) has no such rule); gg_diagnostics reports how
+    many cells hold one: the extrema skip NaNs (fmin / fmax), the sums do not."""
+    wl = workloads.random_problem(12, 200, 90, batch=2)
+    U, V, W = wl.U.copy(), wl.V.copy(), wl.W.copy()
+    W[1, 40, 17] = np.nan
+    U[1, 3, 199] = np.inf
+    V[1, 3, 199] = -np.inf          # same cell: counted once
+    with binding.from_workload(wl) as sim:
+        sim.set_state(U, V, W)
+        got = sim.diagnostics(1e-2)
+        ref = [oracle.diagnostics(U[s], V[s], W[s], 1e-2) for s in range(2)]
+        assert got[0][8] == 0 and got[1][8] == 2
+        check_diag(got[0], ref[0])
+        assert np.isnan(got[1][2]) and got[1][0] == np.inf and got[1][1] == -np.inf
+        assert list(got[1][3:]) == list(ref[1][3:])
+        sim.step(4, wl.dt)          # the NaN spreads one cell per step through W's nine-point stencil
+        after = sim.diagnostics(1e-2)
+        assert after[0][8] == 0 and after[1][8] > 2

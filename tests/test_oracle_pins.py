@@ -470,13 +470,16 @@ def test_diagnostics_brute_force_and_special_cases():
             tum += int(V[j, i] >= 0.5)
             mnw = min(mnw, W[j, i]); mxu = max(mxu, U[j, i]); mxw = max(mxw, W[j, i])
     np.testing.assert_allclose(got[:3], [su, sv, sw], rtol=1e-14)
-    assert (got[3], got[4], got[5], got[6], got[7]) == (gap, tum, mnw, mxu, mxw)
+    assert (got[3], got[4], got[5], got[6], got[7], got[8]) == (gap, tum, mnw, mxu, mxw, 0)
     # the healthy state (1,0,0): no gap, no tumour; the invaded state (0,1,1): no gap, all tumour;
     # (0,0,w): every cell is gap
     n = 12
     one, zero = np.ones((3, 4)), np.zeros((3, 4))
-    assert list(oracle.diagnostics(one, zero, zero, 1e-2)) == [n, 0, 0, 0, 0, 0, 1, 0]
-    assert list(oracle.diagnostics(zero, one, one, 1e-2)) == [0, n, n, 0, n, 1, 0, 1]
+    assert list(oracle.diagnostics(one, zero, zero, 1e-2)) == [n, 0, 0, 0, 0, 0, 1, 0, 0]
+    assert list(oracle.diagnostics(zero, one, one, 1e-2)) == [0, n, n, 0, n, 1, 0, 1, 0]
+    bad = one.copy(); bad[1, 2] = np.nan; bad[0, 0] = np.inf
+    d = oracle.diagnostics(zero, bad, bad * 0.5, 1e-2)     # NaN / Inf cells are counted, extrema skip NaN
+    assert d[8] == 2 and d[5] == 0.5 and d[7] == np.inf and np.isnan(d[1])
     assert oracle.diagnostics(zero, zero, one * 0.3, 1e-2)[3] == n
     # thresholds are strict / inclusive as documented: U == eps is not gap, V == 1/2 is tumour
     assert oracle.diagnostics(one * 1e-2, zero, zero, 1e-2)[3] == 0
