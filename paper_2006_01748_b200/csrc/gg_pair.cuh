@@ -287,7 +287,10 @@ __global__ void __launch_bounds__(256, 1) gg_step_pair(const __grid_constant__ P
                 }
             };
             if (jfirst >= 2 && jfirst + RB - 1 < ny) {
-#pragma unroll
+                // fp32's row body is twice as long per lane (4 cells): unrolling two rows keeps
+                // the hot loop inside the instruction cache (+2 % at 8192^2); fp64 wants all RB
+                constexpr int UNR = sizeof(T) == 4 && RB % 2 == 0 ? 2 : RB;
+#pragma unroll UNR
                 for (int rr = 0; rr < RB; ++rr) row_body(std::false_type{}, rr);
             } else {
 #pragma unroll
