@@ -23,6 +23,7 @@
 #include "gg_diag.cuh"
 #include "gg_pair.cuh"
 #include "gg_quad.cuh"
+#include "gg_quad2.cuh"
 #include "gg_resident.cuh"
 
 namespace {

@@ -1,0 +1,232 @@
+// gg_quad2.cuh -- GG_KERNEL_QUAD, "C" builds: the four-step kernel of gg_quad.cuh with the B warps
+// fetching THEIR OWN coefficient rows by TMA (the rows are L2-hot: the A warps' TMA just read them)
+// instead of receiving copies through ring1.  ring1 then carries U, V, W only, which buys a third
+// ring1 stage (looser coupling between the A and B groups) and takes three of the six shared-memory
+// stores per row off the A warps.  fp64 only (one TMA box per array and row).  Everything else --
+// geometry, barriers, row body, arithmetic -- is gg_quad.cuh's.
+#pragma once
+#include "gg_quad.cuh"
+
+namespace gg {
+
+template <typename T> __host__ __device__ constexpr int quadc_smem_bytes(int rb, int nst0, int nst1, int nstc) {
+    return 256 + nst0 * quad_ring0_stage<T>(rb) + nst1 * (quad_ring1_stage(rb) / 2) +
+           nstc * (quad_ring0_stage<T>(rb) / 2);
+}
+
+// blockDim = 256: warps 0..3 = A, 4..7 = B.  Dynamic shared memory:
+// [full0[NST0], full1[NST1], empty1[NST1], fullC[NSTC] mbarriers, count0[NST0], countC[NSTC];
+//  256 B][ring0: 6 arrays][ringC: a,b,c for the B warps][ring1: U,V,W].
+template <typename T, int RB, int NST0, int NST1, int NSTC>
+__global__ void __launch_bounds__(256, 1) gg_step_quadc(const __grid_constant__ PairArgs A) {
+    constexpr int C = 16 / (int)sizeof(T);
+    constexpr int GW = pair_gw<T>();
+    constexpr int NG = 4 / GW;
+    constexpr int VW = kPairLanes * C;
+    constexpr int BOXB = pair_box_bytes<T>();
+    constexpr int SLAB = pair_slab_bytes(RB, BOXB);
+    constexpr int ARR0 = NG * SLAB, STAGE0 = 6 * ARR0;
+    constexpr int P1 = kQuadRing1Runs * 16, ARR1 = RB * P1, STAGE1 = 3 * ARR1;
+    constexpr int STAGEC = 3 * ARR0;
+    static_assert(NG == 1, "the C builds need one TMA box per array and row (fp64)");
+    static_assert((NST0 + 2 * NST1 + NSTC) * 8 + (NST0 + NSTC) * 4 <= 256, "too many stages");
+
+    extern __shared__ __align__(128) char smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool isA = warp < 4;
+    const int w = warp & 3;
+    const uint32_t full0 = smem_u32(smem), full1 = full0 + 8u * NST0, empty1 = full1 + 8u * NST1;
+    const uint32_t fullC = empty1 + 8u * NST1;
+    unsigned int* count0 = reinterpret_cast<unsigned int*>(smem + 8 * (NST0 + 2 * NST1 + NSTC));
+    unsigned int* countC = count0 + NST0;
+    char* ring0 = smem + 256;
+    char* ringC = ring0 + (size_t)NST0 * STAGE0;      // TMA destinations first: 128-byte aligned
+    char* ring1 = ringC + (size_t)NSTC * STAGEC;
+    const uint32_t ring0_u32 = smem_u32(ring0), ringC_u32 = smem_u32(ringC);
+    const int nx = A.nx, ny = A.ny;
+    const int tile_cells = kQuadRuns * C;
+    constexpr int NBOX = 6 * NG;
+    constexpr uint32_t STAGE_TX = (uint32_t)(NBOX * RB * BOXB);
+
+    auto issue = [&](const PairCursor& pc, uint32_t slot) {
+        const uint32_t bar = full0 + 8u * slot;
+        const uint32_t dst = ring0_u32 + slot * STAGE0;
+        const int y = pc.it.j0 - 4 + pc.q * RB;
+        if (lane == 0) mbar_expect_tx(bar, STAGE_TX);
+        __syncwarp();
+        if (lane < NBOX) {
+            const int f = lane / NG, g = lane - NG * f;
+            const CUtensorMap* map = f == 0 ? &A.mU : f == 1 ? &A.mV : f == 2 ? &A.mW
+                                   : f == 3 ? &A.ma : f == 4 ? &A.mb : &A.mc;
+            tma_load_3d(dst + f * ARR0 + g * SLAB, map, bar, pc.it.i0 - 2 * C + g * GW * VW, y,
+                        f < 3 ? pc.it.sim : 0);
+        }
+    };
+    // the B warps' coefficient rows of the cursor's stage: a, b, c two rows below the A warps' rows
+    auto issueC = [&](const PairCursor& pc, uint32_t slot) {
+        const uint32_t bar = fullC + 8u * slot;
+        const uint32_t dst = ringC_u32 + slot * STAGEC;
+        const int y = pc.it.j0 - 6 + pc.q * RB;
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(3 * RB * BOXB));
+        __syncwarp();
+        if (lane < 3) {
+            const CUtensorMap* map = lane == 0 ? &A.ma : lane == 1 ? &A.mb : &A.mc;
+            tma_load_3d(dst + lane * ARR0, map, bar, pc.it.i0 - 2 * C, y, 0);
+        }
+    };
+    auto advance_cursor = [&](PairCursor& pc) {
+        if (pc.item >= A.nitems) return;
+        if (++pc.q == pc.it.nstage) {
+            pc.q = 0;
+            pc.item += gridDim.x;
+            if (pc.item < A.nitems) pc.it = quad_item<RB>(A, pc.item, tile_cells);
+        }
+    };
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST0; ++s) { mbar_init(full0 + 8u * s, 1); count0[s] = 0u; }
+        for (int s = 0; s < NSTC; ++s) { mbar_init(fullC + 8u * s, 1); countC[s] = 0u; }
+        for (int s = 0; s < NST1; ++s) { mbar_init(full1 + 8u * s, 4); mbar_init(empty1 + 8u * s, 4); }
+        fence_barrier_init();
+        fence_proxy_async();
+    }
+    // ring1 runs that no A lane writes are read (and discarded) by B's outermost lanes
+    for (int o = threadIdx.x * 16; o < NST1 * STAGE1; o += 256 * 16)
+        *reinterpret_cast<uint4*>(ring1 + o) = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
+
+    PairCursor pc;
+    pc.item = blockIdx.x;
+    pc.q = 0;
+    if (pc.item < A.nitems) pc.it = quad_item<RB>(A, pc.item, tile_cells);
+    if (isA) {
+        for (int s = 0; s < NST0; ++s) {
+            if (warp == 0 && pc.item < A.nitems) issue(pc, (uint32_t)s);
+            advance_cursor(pc);
+        }
+    } else {
+        for (int s = 0; s < NSTC; ++s) {
+            if (warp == 4 && pc.item < A.nitems) issueC(pc, (uint32_t)s);
+            advance_cursor(pc);
+        }
+    }
+
+    // where this lane finds its run in a stage of its source ring, and the ring's strides
+    const int src_off = isA ? (w / GW) * SLAB + (w % GW) * (VW * (int)sizeof(T)) + 16 * lane
+                            : (30 * w + lane + 1) * 16;
+    const int src_arr = isA ? ARR0 : ARR1, src_row = isA ? BOXB : P1;
+    // B: own run inside a coefficient box (same origin as ring0's boxes: run -2); the outermost
+    // lane of B warp 3 owns run 120, one past the box: it reads (and discards) the last run
+    const int cof_off = isA ? src_off : min((30 * w + lane + 1) * 16, BOXB - 16);
+    const int dst_off = (30 * w + lane) * 16;              // A: own run in a ring1 row
+    const int run0 = isA ? 30 * w - 2 + lane : 30 * w - 1 + lane;  // tile run this lane owns
+    const bool lane_ok = lane >= 1 && lane <= (isA || w < 3 ? kPairLanes : kPairLanes - 2);
+    const size_t plane = (size_t)nx * ny;
+
+    uint32_t gc = 0;
+    for (long long item = blockIdx.x; item < A.nitems; item += gridDim.x) {
+        const PairItem it = quad_item<RB>(A, item, tile_cells);
+        const int iown = it.i0 + run0 * C;               // first own cell (may lie outside the domain)
+        const bool store_ok = lane_ok && iown >= 0 && iown < nx;
+        const bool atW = iown == 0, atE = iown + C == nx;
+        const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+        T* gU = (T*)A.U1 + it.sim * plane + iown;
+        T* gV = (T*)A.V1 + it.sim * plane + iown;
+        T* gW = (T*)A.W1 + it.sim * plane + iown;
+
+        PairLevel<T, C> L1, L2;
+        L1.clear();
+        L2.clear();
+
+        for (int q = 0; q < it.nstage; ++q, ++gc) {
+            const uint32_t s0 = gc % NST0, s1 = gc % NST1, sc = gc % NSTC;
+            if (isA) {
+                mbar_wait(full0 + 8u * s0, (gc / NST0) & 1u);
+                if (gc >= NST1) mbar_wait(empty1 + 8u * s1, ((gc / NST1) - 1u) & 1u);
+            } else {
+                mbar_wait(fullC + 8u * sc, (gc / NSTC) & 1u);
+                mbar_wait(full1 + 8u * s1, (gc / NST1) & 1u);
+            }
+            // coefficient rows: A finds them in its ring0 stage, B in its own coefficient ring
+            const char* cof = (isA ? ring0 + (size_t)s0 * STAGE0 + 3 * ARR0 : ringC + (size_t)sc * STAGEC) + cof_off;
+            const char* src = (isA ? ring0 + (size_t)s0 * STAGE0 : ring1 + (size_t)s1 * STAGE1) + src_off;
+            char* dst = ring1 + (size_t)s1 * STAGE1 + dst_off;
+            // first row arriving at this role in this stage: time k for A, time k+2 for B
+            const int jfirst = it.j0 - 4 + q * RB - (isA ? 0 : 2);
+            auto row_body = [&](auto ghost_c, const int rr) {
+                constexpr bool GHOST = decltype(ghost_c)::value;
+                const int jn = jfirst + rr;
+                const char* p = src + rr * src_row;
+                T uN[C], vN[C], wN[C], aN[C], bN[C], cN[C];
+                ld_run<T, C>(p + 0 * src_arr, uN);
+                ld_run<T, C>(p + 1 * src_arr, vN);
+                ld_run<T, C>(p + 2 * src_arr, wN);
+                const char* pcf = cof + rr * BOXB;
+                ld_run<T, C>(pcf + 0 * ARR0, aN);
+                ld_run<T, C>(pcf + 1 * ARR0, bN);
+                ld_run<T, C>(pcf + 2 * ARR0, cN);
+                T u1[C], v1[C], w1[C], a1[C], b1[C], c1[C];   // row jn-1, one level up
+                L1.template advance<GHOST>(jn, ny, atW, atE, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
+                T u2[C], v2[C], w2[C], a2[C], b2[C], c2[C];   // row jn-2, two levels up
+                L2.template advance<GHOST>(jn - 1, ny, atW, atE, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
+                if (isA) {
+                    if (lane_ok) {                            // time-k+2 row jn-2 and its coefficients
+                        char* o = dst + rr * P1;
+                        st_run<T, C>(o + 0 * ARR1, u2);
+                        st_run<T, C>(o + 1 * ARR1, v2);
+                        st_run<T, C>(o + 2 * ARR1, w2);
+                    }
+                } else {
+                    const int r = jn - 2;                     // time-k+4 row
+                    if (store_ok && r >= it.j0 && r < it.j1) {
+                        const size_t off = (size_t)r * nx;
+                        st_run<T, C>((char*)(gU + off), u2);
+                        st_run<T, C>((char*)(gV + off), v2);
+                        st_run<T, C>((char*)(gW + off), w2);
+                    }
+                }
+            };
+            if (jfirst >= 2 && jfirst + RB - 1 < ny) {
+#pragma unroll
+                for (int rr = 0; rr < RB; ++rr) row_body(std::false_type{}, rr);
+            } else {
+#pragma unroll
+                for (int rr = 0; rr < RB; ++rr) row_body(std::true_type{}, rr);
+            }
+            __syncwarp();
+            if (isA) {
+                // ring1 stage written (release); ring0 slot read: the A warp that releases it last
+                // refills it with the stage NST0 ahead
+                unsigned int prev = 0;
+                if (lane == 0) {
+                    mbar_arrive(full1 + 8u * s1);
+                    __threadfence_block();
+                    prev = atomicAdd(&count0[s0], 1u);
+                }
+                prev = __shfl_sync(0xffffffffu, prev, 0);
+                if (prev == 3u) {
+                    if (lane == 0) { count0[s0] = 0u; __threadfence_block(); }
+                    if (pc.item < A.nitems) issue(pc, s0);
+                }
+                advance_cursor(pc);
+            } else {
+                // ring1 stage read; coefficient slot read: the B warp that releases it last
+                // refills it with the stage NSTC ahead
+                unsigned int prev = 0;
+                if (lane == 0) {
+                    mbar_arrive(empty1 + 8u * s1);
+                    __threadfence_block();
+                    prev = atomicAdd(&countC[sc], 1u);
+                }
+                prev = __shfl_sync(0xffffffffu, prev, 0);
+                if (prev == 3u) {
+                    if (lane == 0) { countC[sc] = 0u; __threadfence_block(); }
+                    if (pc.item < A.nitems) issueC(pc, sc);
+                }
+                advance_cursor(pc);
+            }
+        }
+    }
+}
+
+}  // namespace gg
