@@ -175,7 +175,10 @@ int resolve_kernel(const gg_ctx* c) {
     // fp64 from mid-size grids up: four steps per launch (measured ahead of the pair kernel from
     // 512^2 to 8192^2 and on batches; a flat ~4.9 us per step below that)
     if (c->dtype == GG_F64 && c->nx >= 236 && cells >= 65536.0) return GG_KERNEL_QUAD;
-    // fp32 (issue-bound with 4 cells per lane): two steps per launch in registers
+    // fp32 (issue-bound with 4 cells per lane): two steps per launch in registers; grids up to
+    // ~1024^2 are still latency-bound per launch and run four steps per launch (768^2: 102 vs 83
+    // GLUPS, 1024^2: 141 vs 115)
+    if (c->dtype == GG_F32 && cells > 262144.0 && cells <= 1572864.0 && c->nx >= 472) return GG_KERNEL_QUAD;
     if (cells > 262144.0 && c->nx >= 240) return GG_KERNEL_PAIR;
     return GG_KERNEL_STREAM2;
 }

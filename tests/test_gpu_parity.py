@@ -396,7 +396,8 @@ def test_user_stream_every_auto_path():
     busy = torch.empty(64 << 20, device="cuda")
     for wl, n, want, dtype in ((workloads.make(0), 40, "resident", "f64"),
                                (workloads.make(1, nx=512, ny=160, steps=1), 24, "quad", "f64"),
-                               (workloads.make(3, nx=2048, ny=160, steps=1), 10, "pair", "f32"),
+                               (workloads.make(3, nx=2048, ny=800, steps=1), 10, "pair", "f32"),
+                               (workloads.make(3, nx=1200, ny=400, steps=1), 12, "quad", "f32"),
                                (workloads.random_problem(3, 41, 23), 9, "generic", "f64")):
         for _ in range(4):
             busy.add_(1.0)                       # unrelated work on the default stream
