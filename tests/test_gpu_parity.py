@@ -40,7 +40,7 @@ def oracle_run(wl, steps):
     return tuple(np.stack([o[f] for o in outs]) for f in range(3))
 
 
-def gpu_run(wl, steps, dtype="f64", kernel=None, options=(), split=None):
+def gpu_run(wl, steps, dtype="f64", kernel=None, options=(), split=None, check_launches=True):
     with binding.from_workload(wl, dtype=dtype) as sim:
         if kernel is not None:
             sim.set_option(binding.GG_OPT_KERNEL, KERNELS[kernel])
@@ -51,7 +51,8 @@ def gpu_run(wl, steps, dtype="f64", kernel=None, options=(), split=None):
         used = sim.kernel
         launches = sim.launches
         out = sim.get_state_numpy()
-    assert launches == expected_launches(used, split or [steps], explicit=kernel is not None)
+    if check_launches:   # (graph chunks shorter than a call split it like separate calls)
+        assert launches == expected_launches(used, split or [steps], explicit=kernel is not None)
     return out, used
 
 
@@ -223,11 +224,21 @@ def test_stream_and_generic_agree_closely():
 # step loop: graphs, ping-pong parity, repeated calls
 # ---------------------------------------------------------------------------------------------
 def test_graph_and_plain_launches_give_identical_bits():
-    wl = workloads.make(0)
-    a, _ = gpu_run(wl, 131, options=[(binding.GG_OPT_GRAPH, 1), (binding.GG_OPT_GRAPH_CHUNK, 16)])
-    b, _ = gpu_run(wl, 131, options=[(binding.GG_OPT_GRAPH, 0)])
-    for x, y in zip(a, b):
-        assert np.array_equal(x, y)
+    """Graph replay (odd chunk lengths, so graphs of 4-, 2- and 1-step launches are mixed) against
+    plain launches, for every multi-launch kernel."""
+    wl = workloads.make(2, nx=520, ny=120, steps=1)
+    ref = None
+    for kernel in ("stream", "stream2", "pair", "quad"):
+        for chunk in (7, 16, 64):
+            a, _ = gpu_run(wl, 131, kernel=kernel, options=[(binding.GG_OPT_GRAPH, 1), (binding.GG_OPT_GRAPH_CHUNK, chunk)],
+                           check_launches=False)
+            ref = a if ref is None else ref
+            for x, y in zip(a, ref):
+                assert np.array_equal(x, y)
+        b, _ = gpu_run(wl, 131, kernel=kernel, options=[(binding.GG_OPT_GRAPH, 0)])
+        for x, y in zip(b, ref):
+            assert np.array_equal(x, y)
+    assert_close(ref, oracle_run(wl, 131), "f64", "graph replay")
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
