@@ -80,14 +80,9 @@ enum {
 enum {
     GG_OPT_KERNEL = 0,      /* one of GG_KERNEL_*                                               */
     GG_OPT_GRAPH = 1,       /* 1 (default): step loop replayed from a cached CUDA graph; 0: plain launches */
-    GG_OPT_GRAPH_CHUNK = 2, /* steps per captured graph (default 64)                            */
-    GG_OPT_STREAM_VARIANT = 3,  /* tuning: which (rows/box, stages, warps/CTA) build of the STREAM
-                                   kernel runs; 0 .. gg_num_stream_variants()-1                  */
-    GG_OPT_ITEMS_PER_WARP = 4,  /* tuning: target work items (row chunk x tile column) per resident CTA */
-    GG_OPT_STREAM_WARPS = 5,    /* tuning: warps (= strips) per CTA: STREAM 1, 2, 4, 8; STREAM2 1, 2, 4; PAIR 1..8; 0 = from nx */
-    GG_OPT_STREAM2_VARIANT = 6, /* tuning: build of the STREAM2 kernel, 0 .. gg_num_stream2_variants()-1; -1 = tuned default */
-    GG_OPT_PAIR_VARIANT = 7,    /* tuning: build of the PAIR kernel, 0 .. gg_num_pair_variants()-1; -1 = tuned default */
-    GG_OPT_QUAD_VARIANT = 8     /* tuning: build of the QUAD kernel, 0 .. gg_num_quad_variants()-1; -1 = tuned default */
+    GG_OPT_GRAPH_CHUNK = 2  /* steps per captured graph (default 64)                            */
+    /* option numbers >= 3 are tuning knobs (which compiled build, warps per CTA, ...); they are
+     * declared in the library's non-installed csrc/gg_tuning.h and are not part of this interface */
 };
 
 /* One simulation.  nx, ny >= 2 cells; h > 0 the mesh size (dx = dy = h);
@@ -126,8 +121,28 @@ int gg_set_tensor(gg_ctx* ctx, const void* a, const void* b, const void* c);
 int gg_set_state(gg_ctx* ctx, const void* U, const void* V, const void* W);
 
 /* n >= 0 explicit Euler steps of eq. (3) with constant step dt > 0.  All
- * three fields advance together from time-k data only.  n == 0 is a no-op. */
+ * three fields advance together from time-k data only.  n == 0 is a no-op.  dt is handed to the
+ * device in front of the step loop and is not part of any cached graph: a new dt on every call
+ * (the paper's host loop) re-captures nothing. */
 int gg_step(gg_ctx* ctx, long long n, double dt);
+
+/* n >= 0 steps with the NON-UNIFORM step size dt_k of PAPER.md:62 ("computed after each iteration
+ * ... to ensure numerical stability"), re-evaluated ON THE DEVICE every `every_k` >= 1 steps with
+ * no host round trip (the paper's steps 3-4, download the results and let the
+ * CPU compute dt_k).  The paper prints no formula; reading A6 is used:
+ *     dt_k = safety * min(dx,dy)^2 / max( lambda_max(A),  max_s alpha_s * max_ij (1 - U^k_s,ij) ),
+ * lambda_max(A) as in gg_max_stable_dt (cached by gg_set_tensor), alpha (1 - U) the largest
+ * diffusivity of the V equation at time level k (eq. (1)); one dt_k for the whole
+ * batch, held for the every_k steps that follow (the last group may be shorter).  safety > 0.
+ * The reductions are exact (max / min), so dt_k is a deterministic function of the stored state.
+ * GG_KERNEL_RESIDENT cannot change dt inside its single launch: GG_ERR_UNSUPPORTED if it was
+ * selected explicitly (AUTO runs STREAM2 on such grids instead).  Enqueues and returns. */
+int gg_step_adaptive(gg_ctx* ctx, long long n, double safety, long long every_k);
+
+/* The device-side clock: simulated time (the sum of the step sizes of all steps since the last
+ * gg_set_state), the step size of the most recent step, and the number of steps since
+ * gg_set_state.  Any of the three pointers may be NULL.  Synchronises the bound stream. */
+int gg_get_clock(gg_ctx* ctx, double* time, double* dt, long long* steps);
 
 /* Copy the current state (after every step issued so far) into DEVICE arrays [nbatch][ny][nx]. */
 int gg_get_state(gg_ctx* ctx, void* U, void* V, void* W);
@@ -171,7 +186,7 @@ int gg_front(gg_ctx* ctx, int field, int axis, int index, double level, int* out
  * ensure numerical stability" and print no formula; reading A6 is used):
  *     *dt = safety * min(dx,dy)^2 / max(max_s alpha_s, lambda_max),
  * lambda_max = max over cells of the larger eigenvalue of [[a,b],[b,c]] (eq. (2)),
- * reduced on the device from the tensor given to gg_set_tensor.  safety <= 1/4 keeps the linear
+ * reduced on the device by gg_set_tensor and cached there (this call reads 8 bytes back).  safety <= 1/4 keeps the linear
  * part L2-stable (max |symbol| <= 8 lambda_max / h^2); BASELINE.json's workloads use 0.2.
  * lambda_max may be NULL.  Synchronises the bound stream. */
 int gg_max_stable_dt(gg_ctx* ctx, double safety, double* dt, double* lambda_max);
@@ -185,11 +200,14 @@ int gg_set_option(gg_ctx* ctx, int option, long long value);
  * gg_launches:    number of step kernels this context has launched so far (graph replays count
  *                 every kernel node; a STREAM2 / PAIR launch advances two steps, a QUAD launch
  *                 four, a RESIDENT launch all n steps of its gg_step call).
+ * gg_graph_captures: number of CUDA graphs this context has captured and instantiated so far (a
+ *                 graph is keyed by length, ping-pong parity, kernel and every_k -- never by dt).
  * gg_last_step_ms: device time of the most recent gg_step call, measured with CUDA events
  *                 recorded on the bound stream around its launches; synchronises on the end
  *                 event.  *ms < 0 if no step has run. */
 int gg_kernel_used(const gg_ctx* ctx);
 long long gg_launches(const gg_ctx* ctx);
+long long gg_graph_captures(const gg_ctx* ctx);
 int gg_last_step_ms(gg_ctx* ctx, float* ms);
 
 /* Synchronises the bound stream, releases graphs and host resources.  The workspace stays the
@@ -200,13 +218,7 @@ int gg_destroy(gg_ctx* ctx);
  * last failing gg_create* on this thread. */
 const char* gg_last_error(const gg_ctx* ctx);
 
-/* Number of STREAM kernel builds selectable with GG_OPT_STREAM_VARIANT. */
-int gg_num_stream_variants(void);
-int gg_num_stream2_variants(void);
-int gg_num_pair_variants(void);
-int gg_num_quad_variants(void);
-
-/* Library version string, e.g. "gg-b200 0.1 sm_100a". */
+/* Library version string, e.g. "gg-b200 0.2 sm_100a". */
 const char* gg_version(void);
 
 #ifdef __cplusplus

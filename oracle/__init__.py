@@ -149,3 +149,60 @@ def front(F, axis: int, index: int, level: float):
     line = F[index, :] if axis == 0 else F[:, index]
     idx = np.nonzero(line >= level)[0]
     return (int(idx[0]), int(idx[-1])) if idx.size else (-1, -1)
+
+
+# ---------------------------------------------------------------------------------------------
+# Non-uniform step size dt_k ("nonuniform step-size dt_k ...
+# computed after each iteration", PAPER.md:127-128 steps 3-4).  Plain NumPy + the C step above.
+#
+# PARITY UNPINNED as far as the RULE goes (reading A6: the paper prints no formula).
+# What IS pinned (tests/test_oracle_pins.py): the rule's arithmetic against worked values and
+# brute-force loops, its reduction to max_stable_dt when the V diffusivity alpha (1 - U) is at its
+# bound alpha, the time loop against `step` with hand-fed step sizes, the clock against sum dt_k.
+# ---------------------------------------------------------------------------------------------
+def adaptive_dt(U, a, b, c, alpha, dx: float, dy: float | None = None, safety: float = 0.2) -> float:
+    """dt_k = safety * min(dx,dy)^2 / max(lambda_max(A), max_s alpha_s * max_ij (1 - U_s,ij)).
+
+    U: [ny][nx] or [batch][ny][nx]; alpha: scalar or [batch].  lambda_max(A) bounds the W
+    diffusion, alpha (1 - U) is the diffusivity of the V equation (eq. (1)) at the
+    current time level; one step size for the whole batch."""
+    if dy is None:
+        dy = dx
+    U = _c(U)
+    if U.ndim == 2:
+        U = U[None]
+    al = np.broadcast_to(np.asarray(alpha, dtype=np.float64), (U.shape[0],))
+    rate = lambda_max(a, b, c)
+    for s in range(U.shape[0]):
+        rate = max(rate, float(al[s] * np.max(1.0 - U[s])))
+    hmin = min(dx, dy)
+    return safety * hmin * hmin / rate
+
+
+def step_adaptive(U, V, W, a, b, c, *, r, d, alpha, c_r, n: int, safety: float, every_k: int,
+                  dx: float, dy: float | None = None, threads: int = 0):
+    """n explicit steps of eq. (3) with dt_k re-evaluated by `adaptive_dt` from the current U
+    before every group of `every_k` steps (the last group may be shorter).  U, V, W:
+    [batch][ny][nx] (or [ny][nx] for one simulation); r, d, alpha, c_r scalars or [batch].
+    Returns (U, V, W, time, dts) with time = sum of all step sizes and dts = the dt_k of every
+    group."""
+    if dy is None:
+        dy = dx
+    single = np.ndim(U) == 2
+    U, V, W = (np.array(x, dtype=np.float64, ndmin=3) for x in (U, V, W))
+    B = U.shape[0]
+    par = [np.broadcast_to(np.asarray(p, dtype=np.float64), (B,)) for p in (r, d, alpha, c_r)]
+    t, left, dts = 0.0, int(n), []
+    while left > 0:
+        g = min(left, int(every_k))
+        dt = adaptive_dt(U, a, b, c, par[2], dx, dy, safety)
+        for s in range(B):
+            U[s], V[s], W[s] = step(U[s], V[s], W[s], a, b, c, r=par[0][s], d=par[1][s],
+                                    alpha=par[2][s], c_r=par[3][s], n=g, dt=dt, dx=dx, dy=dy,
+                                    threads=threads)
+        t += dt * g
+        dts.append(dt)
+        left -= g
+    if single:
+        U, V, W = U[0], V[0], W[0]
+    return U, V, W, t, dts

@@ -47,6 +47,8 @@ SIGNATURES = {
     "gg_set_tensor": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_set_state": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_step": (ctypes.c_int, [_vp, ctypes.c_longlong, ctypes.c_double]),
+    "gg_step_adaptive": (ctypes.c_int, [_vp, ctypes.c_longlong, ctypes.c_double, ctypes.c_longlong]),
+    "gg_get_clock": (ctypes.c_int, [_vp, _dp, _dp, ctypes.POINTER(ctypes.c_longlong)]),
     "gg_get_state": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_set_tensor_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_set_state_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
@@ -58,14 +60,18 @@ SIGNATURES = {
     "gg_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_longlong]),
     "gg_kernel_used": (ctypes.c_int, [_vp]),
     "gg_launches": (ctypes.c_longlong, [_vp]),
+    "gg_graph_captures": (ctypes.c_longlong, [_vp]),
     "gg_last_step_ms": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_float)]),
     "gg_destroy": (ctypes.c_int, [_vp]),
     "gg_last_error": (ctypes.c_char_p, [_vp]),
+    "gg_version": (ctypes.c_char_p, []),
+}
+# tuning entry points of the non-installed csrc/gg_tuning.h (tests force every build through parity)
+TUNING_SIGNATURES = {
     "gg_num_stream_variants": (ctypes.c_int, []),
     "gg_num_stream2_variants": (ctypes.c_int, []),
     "gg_num_pair_variants": (ctypes.c_int, []),
     "gg_num_quad_variants": (ctypes.c_int, []),
-    "gg_version": (ctypes.c_char_p, []),
 }
 
 _lib = None
@@ -86,7 +92,7 @@ def load() -> ctypes.CDLL:
             raise RuntimeError("libgg.so is missing and nvcc is not available to build it; "
                                "there is no CPU fallback")
         lib = ctypes.CDLL(path)
-        for name, (res, args) in SIGNATURES.items():
+        for name, (res, args) in {**SIGNATURES, **TUNING_SIGNATURES}.items():
             fn = getattr(lib, name)
             fn.restype, fn.argtypes = res, args
         _lib = lib
@@ -146,6 +152,17 @@ def gg_step(ctx, n: int, dt: float):
     _check(ctx, load().gg_step(ctx, int(n), float(dt)))
 
 
+def gg_step_adaptive(ctx, n: int, safety: float, every_k: int):
+    _check(ctx, load().gg_step_adaptive(ctx, int(n), float(safety), int(every_k)))
+
+
+def gg_get_clock(ctx):
+    """(time, dt of the most recent step, steps) of the device-side clock."""
+    t, dt, n = ctypes.c_double(0.0), ctypes.c_double(0.0), ctypes.c_longlong(0)
+    _check(ctx, load().gg_get_clock(ctx, ctypes.byref(t), ctypes.byref(dt), ctypes.byref(n)))
+    return float(t.value), float(dt.value), int(n.value)
+
+
 def gg_get_state(ctx, U_ptr, V_ptr, W_ptr):
     _check(ctx, load().gg_get_state(ctx, U_ptr, V_ptr, W_ptr))
 
@@ -199,6 +216,10 @@ def gg_kernel_used(ctx) -> int:
 
 def gg_launches(ctx) -> int:
     return int(load().gg_launches(ctx))
+
+
+def gg_graph_captures(ctx) -> int:
+    return int(load().gg_graph_captures(ctx))
 
 
 def gg_last_step_ms(ctx) -> float:
@@ -292,6 +313,16 @@ class Simulation:
     def step(self, n, dt):
         gg_step(self.ctx, n, dt)
 
+    def step_adaptive(self, n, safety=0.2, every_k=1):
+        gg_step_adaptive(self.ctx, n, safety, every_k)
+
+    def clock(self):
+        return gg_get_clock(self.ctx)
+
+    @property
+    def graph_captures(self) -> int:
+        return gg_graph_captures(self.ctx)
+
     def get_state(self):
         """Current (U, V, W) as device tensors [batch][ny][nx]."""
         sh = (self.batch, self.ny, self.nx)
@@ -343,9 +374,14 @@ class Simulation:
 
     def _after_current_stream(self):
         """libgg enqueues on the bound stream; tensors staged by torch live on torch's current
-        stream: order the bound stream after it (stream plumbing only)."""
+        stream (inputs must be ready there): order the bound stream after it, also when the
+        bound stream is the legacy default stream -- torch side streams are non-blocking and not
+        implicitly ordered with it (stream plumbing only)."""
+        cur = self.torch.cuda.current_stream(self.device)
         if self.stream is not None:
-            self.stream.wait_stream(self.torch.cuda.current_stream(self.device))
+            self.stream.wait_stream(cur)
+        elif int(cur.cuda_stream) != 0:
+            cur.synchronize()
 
     def _sync(self):
         if self.stream is None:

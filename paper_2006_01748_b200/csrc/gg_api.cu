@@ -6,10 +6,12 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <limits>
 #include <map>
 #include <new>
 #include <string>
@@ -23,7 +25,8 @@
 #include "gg_diag.cuh"
 #include "gg_pair.cuh"
 #include "gg_quad.cuh"
-#include "gg_quad2.cuh"
+#include "gg_dt.cuh"
+#include "gg_tuning.h"
 #include "gg_resident.cuh"
 
 namespace {
@@ -33,13 +36,15 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 thread_local std::string g_create_error;
 
+// A captured graph holds step kernels only (plus, for gg_step_adaptive, the device-side dt rule):
+// dt never appears in a kernel argument (gg_dt.cuh), so it is not part of the key.
 struct GraphKey {
     long long len;
-    double dt;
     int parity;
     int kernel;
+    long long every_k;   // 0: fixed dt (gg_step); > 0: dt re-evaluated on the device every_k steps
     bool operator<(const GraphKey& o) const {
-        return std::tie(len, dt, parity, kernel) < std::tie(o.len, o.dt, o.parity, o.kernel);
+        return std::tie(len, parity, kernel, every_k) < std::tie(o.len, o.parity, o.kernel, o.every_k);
     }
 };
 
@@ -57,6 +62,10 @@ struct gg_ctx {
     void* state[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
     void* coef[3] = {nullptr, nullptr, nullptr};
     gg::SimScalars* d_sims = nullptr;
+    gg::StepCoef<double>* d_coefs = nullptr;   // folded on the device from the device-side dt (gg_dt.cuh)
+    gg::DevClock* d_clock = nullptr;
+    double folded_dt = std::numeric_limits<double>::quiet_NaN();  // dt the device's d_coefs were folded with (NaN: unknown)
+    long long graph_captures = 0;
     double* d_scratch = nullptr;
     int cur = 0;  // which ping-pong copy holds the current time level
     // options
@@ -123,7 +132,7 @@ int fail(const gg_ctx* c, int code, const char* fmt, ...) {
     } while (0)
 
 struct Layout {
-    size_t state[2][3], coef[3], sims, scratch, res_halo, res_flags, total;
+    size_t state[2][3], coef[3], sims, coefs, clock, scratch, res_halo, res_flags, total;
 };
 int resident_rows(const gg_ctx* c, int max_slabs);
 size_t resident_halo_bytes(const gg_ctx* c);
@@ -140,6 +149,10 @@ Layout layout_of(const gg_ctx* c) {
     for (int f = 0; f < 3; ++f) { L.coef[f] = off; off += cb; }
     L.sims = off;
     off += align_up((size_t)c->nbatch * sizeof(gg::SimScalars));
+    L.coefs = off;
+    off += align_up((size_t)c->nbatch * sizeof(gg::StepCoef<double>));
+    L.clock = off;
+    off += align_up(sizeof(gg::DevClock));
     L.scratch = off;
     off += align_up(scratch_doubles(c) * sizeof(double));
     // edge-row exchange buffers and step counters of the resident kernel (small grids only)
@@ -156,6 +169,14 @@ Layout layout_of(const gg_ctx* c) {
 
 size_t scratch_doubles(const gg_ctx* c) {
     return (size_t)c->nbatch * gg::kDiagMaxBlocks * gg::kDiagCount + (size_t)c->nbatch * gg::kDiagCount;
+}
+
+// The opt-in dynamic shared-memory limit is an attribute of the FUNCTION (process-wide), while the
+// size a plan asks for depends on its context's shape: always raise it to the device cap, so that
+// contexts of different shapes sharing one instantiation never lower each other's limit.
+constexpr int kMaxDynSmem = 227 * 1024;
+cudaError_t allow_max_smem(const void* fn) {
+    return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
 }
 
 bool stream_shape_ok(const gg_ctx* c) { return ((size_t)c->nx * c->esize()) % 16 == 0; }
@@ -200,7 +221,7 @@ namespace {
 // v = 0 is the build tuned on B200; the others stay selectable through
 // GG_OPT_STREAM_VARIANT for re-tuning.
 struct Variant { int rb, nst; };
-constexpr Variant kVariants[] = {{2, 4}, {4, 2}, {2, 3}, {1, 6}, {1, 8}, {4, 3}, {3, 3}, {3, 2}};
+constexpr Variant kVariants[] = {{2, 4}, {4, 2}};
 constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
 constexpr int kDefaultVariant = 1;
 
@@ -220,20 +241,14 @@ int with_variant(int v, int nw, F&& f) {
     switch (v) {
         case 0: return with_nw<T, 2, 4>(nw, f);
         case 1: return with_nw<T, 4, 2>(nw, f);
-        case 2: return with_nw<T, 2, 3>(nw, f);
-        case 3: return with_nw<T, 1, 6>(nw, f);
-        case 4: return with_nw<T, 1, 8>(nw, f);
-        case 5: return nw <= 4 ? with_nw<T, 4, 3>(nw, f) : -1;  // 8 warps would not fit in smem
-        case 6: return with_nw<T, 3, 3>(nw, f);
-        case 7: return with_nw<T, 3, 2>(nw, f);
     }
     return -1;
 }
 
 // Two-step kernel builds: (rows per box, ring0 stages, ring1 stages); NW in {1, 2, 4} warps per
-// step (so 2*NW + 2 warps per CTA).
+// step (so 2*NW + 2 warps per CTA).  Index 0 is the fp64 default, 1 the fp32 default.
 struct Variant2 { int rb, nst0, nst1; };
-constexpr Variant2 kVariants2[] = {{4, 2, 2}, {2, 4, 3}, {2, 3, 3}, {3, 2, 2}, {2, 3, 2}};
+constexpr Variant2 kVariants2[] = {{4, 2, 2}, {3, 2, 2}};
 constexpr int kNumVariants2 = (int)(sizeof(kVariants2) / sizeof(kVariants2[0]));
 
 template <typename T, int RB, int N0, int N1, typename F>
@@ -249,10 +264,7 @@ template <typename T, typename F>
 int with_variant2(int v, int nw, F&& f) {
     switch (v) {
         case 0: return with_nw2<T, 4, 2, 2>(nw, f);
-        case 1: return with_nw2<T, 2, 4, 3>(nw, f);
-        case 2: return with_nw2<T, 2, 3, 3>(nw, f);
-        case 3: return with_nw2<T, 3, 2, 2>(nw, f);
-        case 4: return with_nw2<T, 2, 3, 2>(nw, f);
+        case 1: return with_nw2<T, 3, 2, 2>(nw, f);
     }
     return -1;
 }
@@ -291,6 +303,33 @@ int make_map(gg_ctx* c, CUtensorMap* m, void* base, int depth, int box_bytes, in
     return GG_OK;
 }
 
+// Row-chunk planner of every tiled kernel: the item schedule is static round-robin over
+// `resident` CTAs, so among chunk counts that give between 1 and 4 x the target items pick the one
+// with the best (wave efficiency) x (useful rows / rows loaded); every chunk loads `halo_rows`
+// extra rows.  No chunk is shorter than 16 rows.
+void plan_chunks(const gg_ctx* c, long long per, long long resident, int halo_rows, int* chunk_rows,
+                 int* nchunks) {
+    const long long max_chunks = (c->ny + 15) / 16;
+    const long long target = (long long)c->opt_items_per_warp * resident;
+    long long best_n = 1;
+    double best_score = -1.0;
+    for (long long n = 1; n <= max_chunks; ++n) {
+        const long long rows = (c->ny + n - 1) / n;
+        const long long nch = (c->ny + rows - 1) / rows;  // chunks actually produced
+        if (nch != n) continue;
+        const long long items = per * nch;
+        if (items > 4 * target && n > 1) break;
+        const long long waves = (items + resident - 1) / resident;
+        // ragged last chunk: the slowest CTA still processes `rows` rows per item
+        const double eff = (double)c->ny * per / ((double)waves * resident * rows);
+        double score = eff * (double)rows / (double)(rows + halo_rows);
+        if (items < target) score *= 0.90 + 0.10 * (double)items / (double)target;  // prefer >= target items
+        if (score > best_score + 1e-9) { best_score = score; best_n = nch; }
+    }
+    *chunk_rows = (int)((c->ny + best_n - 1) / best_n);
+    *nchunks = (c->ny + *chunk_rows - 1) / *chunk_rows;
+}
+
 struct KernelPtr {
     const void** out;
     template <typename T, int RB, int NST, int NW>
@@ -315,7 +354,7 @@ int build_plan(gg_ctx* c, bool two_step) {
     // Tuned on B200 at 8192^2: fp64 runs 4 rows per box with 4 strips per
     // step; fp32 runs 3 rows per box with 2 strips (its row body is twice as long per lane, and
     // the smaller build keeps the three warp roles inside the instruction cache).
-    const int v2 = c->opt_variant2 >= 0 ? c->opt_variant2 : (c->dtype == GG_F64 ? 0 : 3);
+    const int v2 = c->opt_variant2 >= 0 ? c->opt_variant2 : (c->dtype == GG_F64 ? 0 : 1);
     if (two_step) {
         const Variant2 var = kVariants2[v2];
         const int nw_max = c->opt_variant2 < 0 && c->dtype == GG_F32 ? 2 : 4;
@@ -324,7 +363,6 @@ int build_plan(gg_ctx* c, bool two_step) {
     } else {
         const Variant var = kVariants[c->opt_variant];
         if (nw == 0) nw = nstrips >= 8 ? 8 : nstrips >= 4 ? 4 : nstrips >= 2 ? 2 : 1;
-        if (c->opt_variant == 5 && nw > 4) nw = 4;
         P.rb = var.rb; P.nst = var.nst; P.nst1 = 0; P.nw = nw; P.steps = 1;
     }
     const int gw_max = 256 / strip_cells;                 // a TMA box is at most 256 elements wide
@@ -357,36 +395,13 @@ int build_plan(gg_ctx* c, bool two_step) {
     }
     if (rc || !fn) return fail(c, GG_ERR_UNSUPPORTED, "no stream kernel build for this variant with %d warps", nw);
     P.fn = fn;
-    GG_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem));
+    GG_CUDA(c, allow_max_smem(fn));
     int per_sm = 0;
     GG_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, P.block, P.smem));
     if (per_sm < 1) return fail(c, GG_ERR_CUDA, "stream kernel does not fit on an SM");
     const long long resident = (long long)c->num_sms * per_sm;
-    // Row chunks.  The schedule is static round-robin over `resident` CTAs, so the item count
-    // should fill whole waves: among chunk counts that give between 1 and 4*opt items per CTA pick
-    // the one with the best (wave efficiency) x (useful rows / rows loaded), where every chunk
-    // loads two halo rows and recomputes one.  No chunk is shorter than 16 rows.
     P.ntilecols = (nstrips + nw - 1) / nw;
-    const long long per = (long long)P.ntilecols * c->nbatch;
-    const long long max_chunks = (c->ny + 15) / 16;
-    const long long target = (long long)c->opt_items_per_warp * resident;
-    long long best_n = 1;
-    double best_score = -1.0;
-    for (long long n = 1; n <= max_chunks; ++n) {
-        const long long rows = (c->ny + n - 1) / n;
-        const long long nch = (c->ny + rows - 1) / rows;  // chunks actually produced
-        if (nch != n) continue;
-        const long long items = per * nch;
-        if (items > 4 * target && n > 1) break;
-        const long long waves = (items + resident - 1) / resident;
-        // ragged last chunk: the slowest CTA still processes `rows` rows per item
-        const double eff = (double)c->ny * per / ((double)waves * resident * rows);
-        double score = eff * (double)rows / (double)(rows + 2 * P.steps);
-        if (items < target) score *= 0.90 + 0.10 * (double)items / (double)target;  // prefer >= target items
-        if (score > best_score + 1e-9) { best_score = score; best_n = nch; }
-    }
-    P.chunk_rows = (int)((c->ny + best_n - 1) / best_n);
-    P.nchunks = (c->ny + P.chunk_rows - 1) / P.chunk_rows;
+    plan_chunks(c, (long long)P.ntilecols * c->nbatch, resident, 2 * P.steps, &P.chunk_rows, &P.nchunks);
     P.nitems = (long long)P.ntilecols * P.nchunks * c->nbatch;
     P.grid = (int)(P.nitems < resident ? P.nitems : resident);
     ready = true;
@@ -397,14 +412,13 @@ int build_plan(gg_ctx* c, bool two_step) {
 #include "gg_resident_plan.inc"
 
 template <typename T>
-int launch_generic(gg_ctx* c, int src, double dt) {
+int launch_generic(gg_ctx* c, int src) {
     gg::GenericArgs<T> a;
     a.U = (const T*)c->state[src][0]; a.V = (const T*)c->state[src][1]; a.W = (const T*)c->state[src][2];
     a.U1 = (T*)c->state[src ^ 1][0]; a.V1 = (T*)c->state[src ^ 1][1]; a.W1 = (T*)c->state[src ^ 1][2];
     a.a = (const T*)c->coef[0]; a.b = (const T*)c->coef[1]; a.c = (const T*)c->coef[2];
-    a.sims = c->d_sims;
+    a.coefs = c->d_coefs;
     a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
-    a.dt = dt; a.dx = c->dx; a.dy = c->dy;
     dim3 block(64, 4, 1);
     dim3 grid((c->nx + 63) / 64, (c->ny + 3) / 4, c->nbatch);
     gg::gg_step_generic<T><<<grid, block, 0, c->stream>>>(a);
@@ -413,7 +427,7 @@ int launch_generic(gg_ctx* c, int src, double dt) {
 }
 
 // One launch of the single-step or two-step stream kernel from copy `src` into `src^1`.
-int launch_stream(gg_ctx* c, int src, double dt, bool two_step) {
+int launch_stream(gg_ctx* c, int src, bool two_step) {
     const gg::StreamPlan& P = two_step ? c->plan2 : c->plan;
     gg::StreamArgs a;
     a.mU = P.state[src][0]; a.mV = P.state[src][1]; a.mW = P.state[src][2];
@@ -421,48 +435,218 @@ int launch_stream(gg_ctx* c, int src, double dt, bool two_step) {
     a.hU = P.state_halo[src][0]; a.hV = P.state_halo[src][1]; a.hW = P.state_halo[src][2];
     a.ha = P.coef_halo[0]; a.hb = P.coef_halo[1]; a.hc = P.coef_halo[2];
     a.U1 = c->state[src ^ 1][0]; a.V1 = c->state[src ^ 1][1]; a.W1 = c->state[src ^ 1][2];
-    a.sims = c->d_sims;
+    a.coefs = c->d_coefs;
     a.nx = c->nx; a.ny = c->ny; a.nbatch = c->nbatch;
     a.ntilecols = P.ntilecols; a.nchunks = P.nchunks; a.chunk_rows = P.chunk_rows;
     a.nitems = P.nitems;
-    a.dt = dt; a.dx = c->dx; a.dy = c->dy;
     void* params[1] = {&a};
     GG_CUDA(c, cudaLaunchKernel(P.fn, dim3(P.grid), dim3(P.block), params, P.smem, c->stream));
     return GG_OK;
 }
 
 // one step from ping-pong copy `src` into `src^1`
-int launch_step(gg_ctx* c, int kernel, int src, double dt) {
+int launch_step(gg_ctx* c, int kernel, int src) {
     switch (kernel) {
         case GG_KERNEL_GENERIC:
-            return c->dtype == GG_F64 ? launch_generic<double>(c, src, dt)
-                                      : launch_generic<float>(c, src, dt);
+            return c->dtype == GG_F64 ? launch_generic<double>(c, src) : launch_generic<float>(c, src);
         case GG_KERNEL_STREAM:
-            return launch_stream(c, src, dt, false);
+            return launch_stream(c, src, false);
         default:
             return fail(c, GG_ERR_UNSUPPORTED, "kernel %d not available", kernel);
     }
 }
 
-// Enqueue `len` time steps starting from ping-pong copy `src`.  GG_KERNEL_STREAM2 advances two
-// steps per launch and finishes an odd count with one single-step launch.  *nlaunch = kernels
-// launched; every launch flips the ping-pong copy.
-int enqueue_steps(gg_ctx* c, int kernel, int src, long long len, double dt, long long* nlaunch) {
-    long long nl = 0;
+// Enqueue `len` time steps starting from ping-pong copy `src`, with whatever step coefficients
+// the device holds when the kernels run.  GG_KERNEL_STREAM2 / PAIR advance two steps per launch,
+// QUAD four; a remainder ends with shallower launches.  *nlaunch = kernels launched so far in
+// this call (also on failure); every launch flips the ping-pong copy.
+int enqueue_steps(gg_ctx* c, int kernel, int src, long long len, long long* nlaunch) {
     int s = src;
     while (len > 0) {
         int rc;
-        if (kernel == GG_KERNEL_STREAM2 && len >= 2) { rc = launch_stream(c, s, dt, true); len -= 2; }
-        else if (kernel == GG_KERNEL_QUAD && len >= 4) { rc = launch_multi(c, c->quad, s, dt); len -= 4; }
-        else if ((kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) && len >= 2) { rc = launch_pair(c, s, dt); len -= 2; }
-        else if (kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) { rc = launch_stream(c, s, dt, false); len -= 1; }
-        else { rc = launch_step(c, kernel, s, dt); len -= 1; }
+        if (kernel == GG_KERNEL_STREAM2 && len >= 2) { rc = launch_stream(c, s, true); len -= 2; }
+        else if (kernel == GG_KERNEL_QUAD && len >= 4) { rc = launch_multi(c, c->quad, s); len -= 4; }
+        else if ((kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) && len >= 2) { rc = launch_pair(c, s); len -= 2; }
+        else if (kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) { rc = launch_stream(c, s, false); len -= 1; }
+        else { rc = launch_step(c, kernel, s); len -= 1; }
         if (rc) return rc;
         s ^= 1;
-        ++nl;
+        ++*nlaunch;
+    }
+    return GG_OK;
+}
+
+long long launches_for(int kernel, long long len) {
+    if (kernel == GG_KERNEL_QUAD) return len / 4 + ((len % 4) >> 1) + (len & 1);
+    return kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ? len / 2 + (len & 1) : len;
+}
+
+// segment length and block count of the two-stage reductions (gg_diag.cuh, gg_dt.cuh)
+void reduce_geometry(const gg_ctx* c, size_t* seg, int* nblk) {
+    const size_t plane = c->plane();
+    size_t s = (plane + gg::kDiagMaxBlocks - 1) / gg::kDiagMaxBlocks;
+    s = (s + gg::kDiagThreads - 1) / gg::kDiagThreads * gg::kDiagThreads;
+    *seg = s;
+    *nblk = (int)((plane + s - 1) / s);
+}
+
+// The device-side dt rule for the `k` steps that follow (gg_dt.cuh): min U of copy `src` per
+// simulation, then dt_k, the folded coefficients and the clock.  Two small launches.
+int enqueue_adapt(gg_ctx* c, int src, long long k) {
+    size_t seg; int nblk;
+    reduce_geometry(c, &seg, &nblk);
+    dim3 grid(nblk, c->nbatch);
+    if (c->dtype == GG_F64)
+        gg::gg_min_u_partial<double><<<grid, gg::kDiagThreads, 0, c->stream>>>((const double*)c->state[src][0], c->plane(), seg, c->d_scratch);
+    else
+        gg::gg_min_u_partial<float><<<grid, gg::kDiagThreads, 0, c->stream>>>((const float*)c->state[src][0], c->plane(), seg, c->d_scratch);
+    GG_CUDA(c, cudaGetLastError());
+    gg::gg_fold_adaptive<<<1, gg::kDiagThreads, 0, c->stream>>>(c->d_clock, c->d_sims, c->d_coefs, c->d_scratch, nblk,
+                                                              c->nbatch, c->dx, c->dy, k);
+    GG_CUDA(c, cudaGetLastError());
+    return GG_OK;
+}
+
+// `len` steps from copy `src`: every_k == 0 -> plain steps; every_k > 0 -> groups of every_k steps,
+// each preceded by the device-side dt rule.
+int enqueue_span(gg_ctx* c, int kernel, int src, long long len, long long every_k, long long* nlaunch) {
+    if (every_k <= 0) return enqueue_steps(c, kernel, src, len, nlaunch);
+    int s = src;
+    while (len > 0) {
+        const long long g = len < every_k ? len : every_k;
+        int rc = enqueue_adapt(c, s, g);
+        if (rc) return rc;
+        const long long before = *nlaunch;
+        rc = enqueue_steps(c, kernel, s, g, nlaunch);
+        if (rc) return rc;
+        s ^= (int)((*nlaunch - before) & 1);
+        len -= g;
+    }
+    return GG_OK;
+}
+
+// parity flip of `len` steps issued in groups of every_k (0: one group)
+int span_flips(int kernel, long long len, long long every_k, long long* nlaunch) {
+    long long nl = 0;
+    if (every_k <= 0) nl = launches_for(kernel, len);
+    else {
+        nl = (len / every_k) * launches_for(kernel, every_k);
+        if (len % every_k) nl += launches_for(kernel, len % every_k);
     }
     *nlaunch = nl;
+    return (int)(nl & 1);
+}
+
+// Capture a span into an executable graph.
+int capture_graph(gg_ctx* c, int kernel, long long len, long long every_k, int src, cudaGraphExec_t* out) {
+    long long nl = 0;
+    cudaStream_t cap = nullptr;
+    GG_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = c->stream;
+    c->stream = cap;  // the launch functions enqueue on c->stream
+    cudaGraph_t graph = nullptr;
+    int rc = GG_OK;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) {
+        rc = fail(c, GG_ERR_CUDA, "cudaStreamBeginCapture: %s", cudaGetErrorString(e));
+    } else {
+        rc = enqueue_span(c, kernel, src, len, every_k, &nl);
+        e = cudaStreamEndCapture(cap, &graph);
+        if (rc == GG_OK && e != cudaSuccess)
+            rc = fail(c, GG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    }
+    c->stream = user;
+    if (rc == GG_OK) {
+        e = cudaGraphInstantiate(out, graph, 0);
+        if (e != cudaSuccess) rc = fail(c, GG_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+        else ++c->graph_captures;
+    }
+    if (graph) cudaGraphDestroy(graph);
+    cudaStreamDestroy(cap);
+    return rc;
+}
+
+int build_plans(gg_ctx* ctx, int kernel) {
+    int rc = GG_OK;
+    if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ||
+        kernel == GG_KERNEL_QUAD)
+        rc = build_plan(ctx, false);
+    if (!rc && (kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD)) rc = build_plan_pair(ctx);
+    if (!rc && kernel == GG_KERNEL_QUAD) rc = build_plan_quad(ctx);
+    if (!rc && kernel == GG_KERNEL_STREAM2) rc = build_plan(ctx, true);
+    return rc;
+}
+
+// The step loop shared by gg_step (every_k = 0) and gg_step_adaptive: replay cached graphs of up
+// to opt_chunk steps (whole groups of every_k), or plain launches with GG_OPT_GRAPH = 0.
+int run_steps(gg_ctx* ctx, int kernel, long long n, long long every_k) {
+    long long left = n;
+    if (ctx->opt_graph && n >= 2) {
+        long long chunk = ctx->opt_chunk;
+        if (every_k > 0) chunk = chunk / every_k >= 1 ? chunk / every_k * every_k : every_k;
+        while (left > 0) {
+            const long long len = left < chunk ? left : chunk;
+            const GraphKey key{len, ctx->cur, kernel, every_k};
+            auto it = ctx->graphs.find(key);
+            if (it == ctx->graphs.end()) {
+                if (ctx->graphs.size() >= 32) drop_graphs(ctx);
+                cudaGraphExec_t ex = nullptr;
+                int rc = capture_graph(ctx, kernel, len, every_k, ctx->cur, &ex);
+                if (rc) return rc;
+                it = ctx->graphs.emplace(key, ex).first;
+            }
+            GG_CUDA(ctx, cudaGraphLaunch(it->second, ctx->stream));
+            long long nl = 0;
+            ctx->cur ^= span_flips(kernel, len, every_k, &nl);
+            ctx->launches += nl;
+            left -= len;
+        }
+    } else {
+        long long nl = 0;
+        const int rc = enqueue_span(ctx, kernel, ctx->cur, left, every_k, &nl);
+        ctx->cur ^= (int)(nl & 1);
+        ctx->launches += nl;
+        if (rc) {
+            // some launches may have been enqueued: the ping-pong copies no longer hold a
+            // consistent time level
+            ctx->have_state = false;
+            return rc;
+        }
+    }
     return GG_OK;
+}
+
+template <typename T>
+int finish_tensor(gg_ctx* ctx) {
+    // lambda_max(A) of the tensor as given, cached on the device for the step-size rule ...
+    size_t seg; int nblk;
+    reduce_geometry(ctx, &seg, &nblk);
+    gg::gg_lambda_max_partial<T><<<nblk, gg::kDiagThreads, 0, ctx->stream>>>(
+        (const T*)ctx->coef[0], (const T*)ctx->coef[1], (const T*)ctx->coef[2], ctx->plane(), seg, ctx->d_scratch);
+    GG_CUDA(ctx, cudaGetLastError());
+    gg::gg_lambda_final<<<1, gg::kDiagThreads, 0, ctx->stream>>>(ctx->d_scratch, nblk, ctx->d_clock);
+    GG_CUDA(ctx, cudaGetLastError());
+    // ... then a and c in their stored, pre-scaled form (StepCoef comment in gg_common.cuh)
+    const int blocks = (int)std::min<size_t>((ctx->plane() + 255) / 256, (size_t)ctx->num_sms * 8);
+    gg::gg_scale_tensor<T><<<blocks, 256, 0, ctx->stream>>>((const T*)ctx->coef[0], (T*)ctx->coef[0], ctx->plane(),
+                                                           gg::tensor_scale_a(ctx->dx, ctx->dy));
+    GG_CUDA(ctx, cudaGetLastError());
+    gg::gg_scale_tensor<T><<<blocks, 256, 0, ctx->stream>>>((const T*)ctx->coef[2], (T*)ctx->coef[2], ctx->plane(),
+                                                           gg::tensor_scale_c(ctx->dx, ctx->dy));
+    GG_CUDA(ctx, cudaGetLastError());
+    return GG_OK;
+}
+
+// Function-level guard: nothing throws across the ABI (std::bad_alloc from the host containers).
+template <typename F>
+int guarded(const gg_ctx* c, const char* what, F&& f) {
+    try {
+        return f();
+    } catch (const std::bad_alloc&) {
+        try { return fail(c, GG_ERR_ARG, "%s: out of host memory", what); } catch (...) { return GG_ERR_ARG; }
+    } catch (...) {
+        try { return fail(c, GG_ERR_CUDA, "%s: unexpected C++ exception", what); } catch (...) { return GG_ERR_CUDA; }
+    }
 }
 
 }  // namespace
@@ -474,26 +658,36 @@ extern "C" {
 
 int gg_create_xy(gg_ctx** out, int nbatch, int nx, int ny, double dx, double dy, const double* r,
                  const double* d, const double* alpha, const double* c, int dtype) {
-    if (!out) return fail(nullptr, GG_ERR_ARG, "gg_create: out is NULL");
-    *out = nullptr;
-    if (nbatch < 1) return fail(nullptr, GG_ERR_ARG, "gg_create: nbatch %d < 1", nbatch);
-    if (nx < 2 || ny < 2) return fail(nullptr, GG_ERR_ARG, "gg_create: nx, ny must be >= 2 (got %d x %d)", nx, ny);
-    if (!(dx > 0.0) || !std::isfinite(dx) || !(dy > 0.0) || !std::isfinite(dy))
-        return fail(nullptr, GG_ERR_ARG, "gg_create: mesh sizes must be finite and > 0");
-    if (!r || !d || !alpha || !c) return fail(nullptr, GG_ERR_ARG, "gg_create: NULL parameter array");
-    if (dtype != GG_F64 && dtype != GG_F32) return fail(nullptr, GG_ERR_UNSUPPORTED, "gg_create: unknown dtype %d", dtype);
-    if ((double)nx * ny * nbatch > 2.0e10) return fail(nullptr, GG_ERR_ARG, "gg_create: grid too large");
-    for (int s = 0; s < nbatch; ++s)
-        if (!std::isfinite(r[s]) || !std::isfinite(d[s]) || !std::isfinite(alpha[s]) || !std::isfinite(c[s]))
-            return fail(nullptr, GG_ERR_ARG, "gg_create: non-finite parameter for simulation %d", s);
-    gg_ctx* ctx = new (std::nothrow) gg_ctx;
-    if (!ctx) return fail(nullptr, GG_ERR_ARG, "gg_create: out of host memory");
-    ctx->nx = nx; ctx->ny = ny; ctx->nbatch = nbatch; ctx->dx = dx; ctx->dy = dy; ctx->dtype = dtype;
-    ctx->sims.resize(nbatch);
-    for (int s = 0; s < nbatch; ++s) ctx->sims[s] = gg::SimScalars{r[s], d[s], alpha[s], c[s]};
-    ctx->opt_variant = kDefaultVariant;
-    *out = ctx;
-    return GG_OK;
+    return guarded(nullptr, "gg_create", [&]() -> int {
+        if (!out) return fail(nullptr, GG_ERR_ARG, "gg_create: out is NULL");
+        *out = nullptr;
+        if (nbatch < 1) return fail(nullptr, GG_ERR_ARG, "gg_create: nbatch %d < 1", nbatch);
+        if (nx < 2 || ny < 2) return fail(nullptr, GG_ERR_ARG, "gg_create: nx, ny must be >= 2 (got %d x %d)", nx, ny);
+        // launch-geometry limits of the one-thread-per-cell and reduction kernels (gridDim.y / .z)
+        if (nbatch > 65535) return fail(nullptr, GG_ERR_ARG, "gg_create: nbatch %d > 65535", nbatch);
+        if (ny > 262140) return fail(nullptr, GG_ERR_ARG, "gg_create: ny %d > 262140", ny);
+        if (!(dx > 0.0) || !std::isfinite(dx) || !(dy > 0.0) || !std::isfinite(dy))
+            return fail(nullptr, GG_ERR_ARG, "gg_create: mesh sizes must be finite and > 0");
+        if (!r || !d || !alpha || !c) return fail(nullptr, GG_ERR_ARG, "gg_create: NULL parameter array");
+        if (dtype != GG_F64 && dtype != GG_F32) return fail(nullptr, GG_ERR_UNSUPPORTED, "gg_create: unknown dtype %d", dtype);
+        if ((double)nx * ny * nbatch > 2.0e10) return fail(nullptr, GG_ERR_ARG, "gg_create: grid too large");
+        for (int s = 0; s < nbatch; ++s)
+            if (!std::isfinite(r[s]) || !std::isfinite(d[s]) || !std::isfinite(alpha[s]) || !std::isfinite(c[s]))
+                return fail(nullptr, GG_ERR_ARG, "gg_create: non-finite parameter for simulation %d", s);
+        gg_ctx* ctx = new (std::nothrow) gg_ctx;
+        if (!ctx) return fail(nullptr, GG_ERR_ARG, "gg_create: out of host memory");
+        ctx->nx = nx; ctx->ny = ny; ctx->nbatch = nbatch; ctx->dx = dx; ctx->dy = dy; ctx->dtype = dtype;
+        try {
+            ctx->sims.resize(nbatch);
+        } catch (...) {
+            delete ctx;
+            throw;
+        }
+        for (int s = 0; s < nbatch; ++s) ctx->sims[s] = gg::SimScalars{r[s], d[s], alpha[s], c[s]};
+        ctx->opt_variant = kDefaultVariant;
+        *out = ctx;
+        return GG_OK;
+    });
 }
 
 int gg_create_batch(gg_ctx** out, int nbatch, int nx, int ny, double h, const double* r,
@@ -527,11 +721,14 @@ int gg_bind(gg_ctx* ctx, void* ws, size_t bytes, void* stream) {
         for (int f = 0; f < 3; ++f) ctx->state[p][f] = ctx->ws + L.state[p][f];
     for (int f = 0; f < 3; ++f) ctx->coef[f] = ctx->ws + L.coef[f];
     ctx->d_sims = (gg::SimScalars*)(ctx->ws + L.sims);
+    ctx->d_coefs = (gg::StepCoef<double>*)(ctx->ws + L.coefs);
+    ctx->d_clock = (gg::DevClock*)(ctx->ws + L.clock);
     ctx->d_scratch = (double*)(ctx->ws + L.scratch);
     if (L.res_halo) {
         ctx->d_res_halo = ctx->ws + L.res_halo;
         ctx->d_res_flags = (unsigned int*)(ctx->ws + L.res_flags);
     }
+    GG_CUDA(ctx, cudaMemsetAsync(ctx->d_clock, 0, sizeof(gg::DevClock), ctx->stream));
     GG_CUDA(ctx, cudaMemcpyAsync(ctx->d_sims, ctx->sims.data(), ctx->sims.size() * sizeof(gg::SimScalars),
                                  cudaMemcpyHostToDevice, ctx->stream));
     GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // sims is pageable host memory
@@ -554,8 +751,11 @@ static int set_tensor_impl(gg_ctx* ctx, const void* a, const void* b, const void
     if (!ctx->bound) return fail(ctx, GG_ERR_STATE, "gg_set_tensor: call gg_bind first");
     if (!a || !b || !c) return fail(ctx, GG_ERR_ARG, "gg_set_tensor: NULL array");
     const void* src[3] = {a, b, c};
+    ctx->have_tensor = false;
     int rc = copy3(ctx, ctx->coef, src, ctx->plane() * ctx->esize(),
                    host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, host);
+    if (rc) return rc;
+    rc = ctx->dtype == GG_F64 ? finish_tensor<double>(ctx) : finish_tensor<float>(ctx);
     if (rc) return rc;
     ctx->have_tensor = true;
     return GG_OK;
@@ -568,6 +768,8 @@ static int set_state_impl(gg_ctx* ctx, const void* U, const void* V, const void*
     int rc = copy3(ctx, ctx->state[ctx->cur], src, (size_t)ctx->nbatch * ctx->plane() * ctx->esize(),
                    host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, host);
     if (rc) return rc;
+    gg::gg_clock_reset<<<1, 1, 0, ctx->stream>>>(ctx->d_clock);
+    GG_CUDA(ctx, cudaGetLastError());
     ctx->have_state = true;
     return GG_OK;
 }
@@ -587,114 +789,88 @@ int gg_set_state_host(gg_ctx* c, const void* U, const void* V, const void* W) { 
 int gg_get_state(gg_ctx* c, void* U, void* V, void* W) { return get_state_impl(c, U, V, W, false); }
 int gg_get_state_host(gg_ctx* c, void* U, void* V, void* W) { return get_state_impl(c, U, V, W, true); }
 
-}  // extern "C"
-
-namespace {
-
-// Capture `len` consecutive steps starting from ping-pong copy `src` into an executable graph.
-int capture_graph(gg_ctx* c, int kernel, long long len, double dt, int src, cudaGraphExec_t* out) {
-    long long nl = 0;
-    cudaStream_t cap = nullptr;
-    GG_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
-    cudaStream_t user = c->stream;
-    c->stream = cap;  // launch_step enqueues on c->stream
-    cudaGraph_t graph = nullptr;
-    int rc = GG_OK;
-    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
-    if (e != cudaSuccess) {
-        rc = fail(c, GG_ERR_CUDA, "cudaStreamBeginCapture: %s", cudaGetErrorString(e));
-    } else {
-        rc = enqueue_steps(c, kernel, src, len, dt, &nl);
-        e = cudaStreamEndCapture(cap, &graph);
-        if (rc == GG_OK && e != cudaSuccess)
-            rc = fail(c, GG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
-    }
-    c->stream = user;
-    if (rc == GG_OK) {
-        e = cudaGraphInstantiate(out, graph, 0);
-        if (e != cudaSuccess) rc = fail(c, GG_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
-    }
-    if (graph) cudaGraphDestroy(graph);
-    cudaStreamDestroy(cap);
-    return rc;
-}
-
-}  // namespace
-
-extern "C" {
-
 int gg_step(gg_ctx* ctx, long long n, double dt) {
     if (!ctx) return GG_ERR_ARG;
-    if (!ctx->bound || !ctx->have_tensor || !ctx->have_state)
-        return fail(ctx, GG_ERR_STATE, "gg_step: needs gg_bind, gg_set_tensor and gg_set_state first");
-    if (n < 0) return fail(ctx, GG_ERR_ARG, "gg_step: n = %lld < 0", n);
-    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
-    if (n == 0) return GG_OK;
-    int kernel = resolve_kernel(ctx);
-    if (kernel == GG_KERNEL_RESIDENT && ctx->opt_kernel == GG_KERNEL_AUTO && n < kResidentMinSteps)
-        kernel = GG_KERNEL_STREAM2;   // a cooperative launch does not pay for a handful of steps
-    if (kernel == GG_KERNEL_RESIDENT) {
-        int rc = build_plan_resident(ctx);
-        if (rc) return rc;
+    return guarded(ctx, "gg_step", [&]() -> int {
+        if (!ctx->bound || !ctx->have_tensor || !ctx->have_state)
+            return fail(ctx, GG_ERR_STATE, "gg_step: needs gg_bind, gg_set_tensor and gg_set_state first");
+        if (n < 0) return fail(ctx, GG_ERR_ARG, "gg_step: n = %lld < 0", n);
+        if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
+        if (n == 0) return GG_OK;
+        int kernel = resolve_kernel(ctx);
+        const bool autosel = ctx->opt_kernel == GG_KERNEL_AUTO;
+        if (kernel == GG_KERNEL_RESIDENT && autosel && n < kResidentMinSteps)
+            kernel = GG_KERNEL_STREAM2;   // a cooperative launch does not pay for a handful of steps
+        if (kernel == GG_KERNEL_RESIDENT) {
+            const int rc = build_plan_resident(ctx);
+            if (rc && !autosel) return rc;
+            if (rc) kernel = GG_KERNEL_STREAM2;   // AUTO: a refused cooperative plan is not an error
+        }
+        if (kernel != GG_KERNEL_RESIDENT) {
+            const int rc = build_plans(ctx, kernel);
+            if (rc) return rc;
+        }
         GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-        rc = launch_resident(ctx, ctx->cur, n, dt);
-        if (rc) return rc;
-        ctx->cur ^= 1;
-        ctx->launches += 1;
+        // dt goes to the device by value, in front of (never inside) the replayed graphs
+        gg::gg_fold_fixed<<<(ctx->nbatch + 127) / 128, 128, 0, ctx->stream>>>(
+            ctx->d_clock, ctx->d_sims, ctx->d_coefs, ctx->nbatch, dt, ctx->dx, ctx->dy, n,
+            ctx->folded_dt == dt ? 0 : 1);
+        GG_CUDA(ctx, cudaGetLastError());
+        ctx->folded_dt = dt;
+        if (kernel == GG_KERNEL_RESIDENT) {
+            const int rc = launch_resident(ctx, ctx->cur, n);
+            if (rc) return rc;
+            ctx->cur ^= 1;
+            ctx->launches += 1;
+        } else {
+            const int rc = run_steps(ctx, kernel, n, 0);
+            if (rc) return rc;
+        }
         GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
         ctx->timed = true;
         return GG_OK;
-    }
-    if (kernel == GG_KERNEL_STREAM || kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ||
-        kernel == GG_KERNEL_QUAD) {
-        int rc = build_plan(ctx, false);
-        if (rc) return rc;
-    }
-    if (kernel == GG_KERNEL_PAIR || kernel == GG_KERNEL_QUAD) {
-        int rc = build_plan_pair(ctx);
-        if (rc) return rc;
-    }
-    if (kernel == GG_KERNEL_QUAD) {
-        int rc = build_plan_quad(ctx);
-        if (rc) return rc;
-    }
-    if (kernel == GG_KERNEL_STREAM2) {
-        int rc = build_plan(ctx, true);
-        if (rc) return rc;
-    }
-    auto launches_for = [kernel](long long len) {
-        if (kernel == GG_KERNEL_QUAD) return len / 4 + ((len % 4) >> 1) + (len & 1);
-        return kernel == GG_KERNEL_STREAM2 || kernel == GG_KERNEL_PAIR ? len / 2 + (len & 1) : len;
-    };
-    GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-    long long left = n;
-    if (ctx->opt_graph && n >= 2) {
-        const long long chunk = ctx->opt_chunk;
-        while (left > 0) {
-            const long long len = left < chunk ? left : chunk;
-            const GraphKey key{len, dt, ctx->cur, kernel};
-            auto it = ctx->graphs.find(key);
-            if (it == ctx->graphs.end()) {
-                if (ctx->graphs.size() >= 32) drop_graphs(ctx);
-                cudaGraphExec_t ex = nullptr;
-                int rc = capture_graph(ctx, kernel, len, dt, ctx->cur, &ex);
-                if (rc) return rc;
-                it = ctx->graphs.emplace(key, ex).first;
-            }
-            GG_CUDA(ctx, cudaGraphLaunch(it->second, ctx->stream));
-            ctx->cur ^= (int)(launches_for(len) & 1);
-            ctx->launches += launches_for(len);
-            left -= len;
+    });
+}
+
+int gg_step_adaptive(gg_ctx* ctx, long long n, double safety, long long every_k) {
+    if (!ctx) return GG_ERR_ARG;
+    return guarded(ctx, "gg_step_adaptive", [&]() -> int {
+        if (!ctx->bound || !ctx->have_tensor || !ctx->have_state)
+            return fail(ctx, GG_ERR_STATE, "gg_step_adaptive: needs gg_bind, gg_set_tensor and gg_set_state first");
+        if (n < 0) return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: n = %lld < 0", n);
+        if (!(safety > 0.0) || !std::isfinite(safety)) return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: safety must be finite and > 0");
+        if (every_k < 1 || every_k > 4096) return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: every_k must be in 1..4096");
+        if (n == 0) return GG_OK;
+        int kernel = resolve_kernel(ctx);
+        if (kernel == GG_KERNEL_RESIDENT) {
+            // the on-chip kernel advances a whole call in one launch and cannot re-read dt
+            if (ctx->opt_kernel != GG_KERNEL_AUTO)
+                return fail(ctx, GG_ERR_UNSUPPORTED, "gg_step_adaptive: GG_KERNEL_RESIDENT cannot change dt inside its launch");
+            kernel = GG_KERNEL_STREAM2;
         }
-    } else {
-        long long nl = 0;
-        int rc = enqueue_steps(ctx, kernel, ctx->cur, left, dt, &nl);
+        int rc = build_plans(ctx, kernel);
         if (rc) return rc;
-        ctx->cur ^= (int)(nl & 1);
-        ctx->launches += nl;
-    }
-    GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
-    ctx->timed = true;
+        GG_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+        gg::gg_clock_safety<<<1, 1, 0, ctx->stream>>>(ctx->d_clock, safety);
+        GG_CUDA(ctx, cudaGetLastError());
+        ctx->folded_dt = std::numeric_limits<double>::quiet_NaN();   // the device decides from here on
+        rc = run_steps(ctx, kernel, n, every_k);
+        if (rc) return rc;
+        GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+        ctx->timed = true;
+        return GG_OK;
+    });
+}
+
+int gg_get_clock(gg_ctx* ctx, double* time, double* dt, long long* steps) {
+    if (!ctx) return GG_ERR_ARG;
+    if (!ctx->bound) return fail(ctx, GG_ERR_STATE, "gg_get_clock: call gg_bind first");
+    gg::DevClock h;
+    GG_CUDA(ctx, cudaMemcpyAsync(&h, ctx->d_clock, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (time) *time = h.time;
+    if (dt) *dt = h.dt;
+    if (steps) *steps = h.steps;
     return GG_OK;
 }
 
@@ -764,10 +940,8 @@ int gg_diagnostics(gg_ctx* ctx, double eps, double* out) {
     if (!out) return fail(ctx, GG_ERR_ARG, "gg_diagnostics: out is NULL");
     if (!(eps >= 0.0) || !std::isfinite(eps)) return fail(ctx, GG_ERR_ARG, "gg_diagnostics: eps must be finite and >= 0");
     const size_t plane = ctx->plane();
-    // segment per block: a multiple of the block size, at most kDiagMaxBlocks blocks per simulation
-    size_t seg = (plane + gg::kDiagMaxBlocks - 1) / gg::kDiagMaxBlocks;
-    seg = (seg + gg::kDiagThreads - 1) / gg::kDiagThreads * gg::kDiagThreads;
-    const int nblk = (int)((plane + seg - 1) / seg);
+    size_t seg; int nblk;
+    reduce_geometry(ctx, &seg, &nblk);
     double* partial = ctx->d_scratch;
     double* fin = ctx->d_scratch + (size_t)ctx->nbatch * gg::kDiagMaxBlocks * gg::kDiagCount;
     void* const* st = ctx->state[ctx->cur];
@@ -817,22 +991,11 @@ int gg_max_stable_dt(gg_ctx* ctx, double safety, double* dt, double* lambda_max)
     if (!ctx->bound || !ctx->have_tensor) return fail(ctx, GG_ERR_STATE, "gg_max_stable_dt: no tensor set");
     if (!dt) return fail(ctx, GG_ERR_ARG, "gg_max_stable_dt: dt is NULL");
     if (!(safety > 0.0) || !std::isfinite(safety)) return fail(ctx, GG_ERR_ARG, "gg_max_stable_dt: safety must be finite and > 0");
-    const size_t plane = ctx->plane();
-    size_t seg = (plane + gg::kDiagMaxBlocks - 1) / gg::kDiagMaxBlocks;
-    seg = (seg + gg::kDiagThreads - 1) / gg::kDiagThreads * gg::kDiagThreads;
-    const int nblk = (int)((plane + seg - 1) / seg);
-    if (ctx->dtype == GG_F64)
-        gg::gg_lambda_max_partial<double><<<nblk, gg::kDiagThreads, 0, ctx->stream>>>(
-            (const double*)ctx->coef[0], (const double*)ctx->coef[1], (const double*)ctx->coef[2], plane, seg, ctx->d_scratch);
-    else
-        gg::gg_lambda_max_partial<float><<<nblk, gg::kDiagThreads, 0, ctx->stream>>>(
-            (const float*)ctx->coef[0], (const float*)ctx->coef[1], (const float*)ctx->coef[2], plane, seg, ctx->d_scratch);
-    GG_CUDA(ctx, cudaGetLastError());
-    double part[gg::kDiagMaxBlocks];
-    GG_CUDA(ctx, cudaMemcpyAsync(part, ctx->d_scratch, nblk * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    // lambda_max(A) was reduced on the device by gg_set_tensor and is cached in the device clock
+    gg::DevClock h;
+    GG_CUDA(ctx, cudaMemcpyAsync(&h, ctx->d_clock, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
     GG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    double lam = part[0];
-    for (int q = 1; q < nblk; ++q) lam = part[q] > lam ? part[q] : lam;
+    const double lam = h.lambda_max;
     double amax = ctx->sims[0].alpha;
     for (const auto& sc : ctx->sims) amax = sc.alpha > amax ? sc.alpha : amax;
     const double rate = lam > amax ? lam : amax;
@@ -846,6 +1009,7 @@ int gg_max_stable_dt(gg_ctx* ctx, double safety, double* dt, double* lambda_max)
 
 int gg_kernel_used(const gg_ctx* ctx) { return ctx ? resolve_kernel(ctx) : -1; }
 long long gg_launches(const gg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+long long gg_graph_captures(const gg_ctx* ctx) { return ctx ? ctx->graph_captures : 0; }
 
 int gg_last_step_ms(gg_ctx* ctx, float* ms) {
     if (!ctx || !ms) return GG_ERR_ARG;
@@ -874,6 +1038,6 @@ int gg_num_stream_variants(void) { return kNumVariants; }
 int gg_num_stream2_variants(void) { return kNumVariants2; }
 int gg_num_pair_variants(void) { return kNumPairVariants; }
 int gg_num_quad_variants(void) { return kNumQuadVariants; }
-const char* gg_version(void) { return "gg-b200 0.1 sm_100a"; }
+const char* gg_version(void) { return "gg-b200 0.2 sm_100a"; }
 
 }  // extern "C"

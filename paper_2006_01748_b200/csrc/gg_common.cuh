@@ -4,7 +4,8 @@
 // Scheme: eq. (3) of arXiv 2006.01748 with the stencils of Table 1
 // and Table 2, evaluated in FLUX FORM:
 //
-//   (the code carries 2 phi and 2 F and halves the step coefficients instead, see flux_V)
+//   (the code carries 2 phi and pre-scaled 2 F and folds the factors into the step coefficients and
+//    the stored tensor entries instead, see StepCoef and flux_V)
 //   V face flux   phiE_ij = (1 - (U_ij + U_i+1,j)/2) (V_i+1,j - V_ij)          [Table 1, E entry x h^2]
 //                 phiN_ij = (1 - (U_ij + U_i,j+1)/2) (V_i,j+1 - V_ij)
 //   W cross terms G_ij = b_ij (W_i,j+1 - W_i,j-1),  H_ij = b_ij (W_i+1,j - W_i-1,j)
@@ -28,34 +29,52 @@ struct SimScalars {
     double r, d, alpha, c_r;
 };
 
-// Step coefficients in the arithmetic type T.
+// Step coefficients of one simulation.  They live in the workspace as StepCoef<double>, written
+// by the device-side fold kernel (gg_dt.cuh) from the step size that is current ON THE DEVICE, so
+// that neither a new dt nor an adaptive dt_k changes a kernel argument (a captured graph survives
+// any dt).  The step kernels load them and round once to the arithmetic type T.
+//
+// The tensor fields are stored PRE-SCALED (gg_set_tensor): a' = a * 2dy/dx, c' = c * 2dx/dy, b as
+// given.  With G = b (W_i,j+1 - W_i,j-1), H = b (W_i+1,j - W_i-1,j) the doubled W face fluxes of the
+// header comment, divided by the cross-term weights dx/(2dy) resp. dy/(2dx), become
+//     FE' = (a'_ij + a'_i+1,j)(W_i+1,j - W_ij) + (G_ij + G_i+1,j)
+//     FN' = (c'_ij + c'_i,j+1)(W_i,j+1 - W_ij) + (H_ij + H_i,j+1)
+// and both carry the same step weight dt/(4 dx dy): one multiplication less per face, and on a
+// square mesh (2dy/dx = 2) bit-for-bit the values of the unscaled form.
 template <typename T>
 struct StepCoef {
     T dt;     // dt
     T ddt;    // d * dt
     T rdt;    // r * dt
-    T adx;    // alpha * dt / (2 dx^2)   (the face fluxes carry a factor 2, see flux_V)
+    T adx;    // alpha * dt / (2 dx^2)   (the V face fluxes carry a factor 2, see flux_V)
     T ady;    // alpha * dt / (2 dy^2)
     T crdt;   // c_r * dt
-    T sx;     // dt / (2 dx^2)
-    T sy;     // dt / (2 dy^2)
-    T thx;    // dx / (2 dy): weight of the cross terms G in an x-face flux (1/2 on a square mesh)
-    T thy;    // dy / (2 dx): weight of the cross terms H in a y-face flux
+    T sw;     // dt / (4 dx dy): weight of the pre-scaled W face fluxes FE', FN'
+    T pad_;
 };
 
+__host__ __device__ __forceinline__ StepCoef<double> fold_coef(const SimScalars& p, double dt, double dx, double dy) {
+    StepCoef<double> k;
+    k.dt = dt;
+    k.ddt = p.d * dt;
+    k.rdt = p.r * dt;
+    k.adx = 0.5 * p.alpha * dt / (dx * dx);
+    k.ady = 0.5 * p.alpha * dt / (dy * dy);
+    k.crdt = p.c_r * dt;
+    k.sw = 0.25 * dt / (dx * dy);
+    k.pad_ = 0.0;
+    return k;
+}
+// factors the tensor entries a and c are stored with (see above)
+__host__ __device__ __forceinline__ double tensor_scale_a(double dx, double dy) { return 2.0 * dy / dx; }
+__host__ __device__ __forceinline__ double tensor_scale_c(double dx, double dy) { return 2.0 * dx / dy; }
+
 template <typename T>
-__device__ __forceinline__ StepCoef<T> fold_coef(const SimScalars& p, double dt, double dx, double dy) {
+__device__ __forceinline__ StepCoef<T> load_coef(const StepCoef<double>* __restrict__ p) {
+    const StepCoef<double> c = *p;
     StepCoef<T> k;
-    k.dt = (T)dt;
-    k.ddt = (T)(p.d * dt);
-    k.rdt = (T)(p.r * dt);
-    k.adx = (T)(0.5 * p.alpha * dt / (dx * dx));
-    k.ady = (T)(0.5 * p.alpha * dt / (dy * dy));
-    k.crdt = (T)(p.c_r * dt);
-    k.sx = (T)(0.5 * dt / (dx * dx));
-    k.sy = (T)(0.5 * dt / (dy * dy));
-    k.thx = (T)(0.5 * dx / dy);
-    k.thy = (T)(0.5 * dy / dx);
+    k.dt = (T)c.dt; k.ddt = (T)c.ddt; k.rdt = (T)c.rdt; k.adx = (T)c.adx; k.ady = (T)c.ady;
+    k.crdt = (T)c.crdt; k.sw = (T)c.sw; k.pad_ = (T)0;
     return k;
 }
 
@@ -73,8 +92,8 @@ __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b);
 __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 
-// Face fluxes carry a common factor 2 (flux_V = 2 phi, flux_W = 2 F) that fold_coef puts into
-// adt and s: one multiplication less per face.
+// Face fluxes carry a common factor (flux_V = 2 phi, flux_W = 2 F / cross-term weight) that
+// fold_coef puts into adx, ady and sw: fewer multiplications per face.
 template <typename T>
 __device__ __forceinline__ T upd_U(const StepCoef<T>& k, T u, T w) {
     // eq. (3) line 1: U + dt U (1-U) - d dt U W  =  U + U (dt (1-U) - d dt W)
@@ -88,7 +107,7 @@ __device__ __forceinline__ T upd_V(const StepCoef<T>& k, T v, T fe, T fw, T fn, 
 template <typename T>
 __device__ __forceinline__ T upd_W(const StepCoef<T>& k, T v, T w, T fe, T fw, T fn, T fs) {
     // eq. (3) line 3
-    return fma_(k.sx, sub(fe, fw), fma_(k.sy, sub(fn, fs), fma_(k.crdt, sub(v, w), w)));
+    return fma_(k.sw, sub(fe, fw), fma_(k.sw, sub(fn, fs), fma_(k.crdt, sub(v, w), w)));
 }
 template <typename T>
 __device__ __forceinline__ T flux_V(T u0, T u1, T v0, T v1) {
@@ -96,11 +115,10 @@ __device__ __forceinline__ T flux_V(T u0, T u1, T v0, T v1) {
     return mul(sub((T)2, add(u0, u1)), sub(v1, v0));
 }
 template <typename T>
-__device__ __forceinline__ T flux_W(T k0, T k1, T w0, T w1, T x0, T x1, T th) {
-    // 2 dn x [face-mean diffusivity x normal gradient + mean of the two cross terms] (Table 2):
-    // (k0+k1)(w1-w0) + th (x0+x1), x = b x (tangential difference of W), th = dn/(2 dt_) with dn
-    // the mesh size normal to the face and dt_ the tangential one (1/2 on a square mesh)
-    return fma_(add(k0, k1), sub(w1, w0), mul(th, add(x0, x1)));
+__device__ __forceinline__ T flux_W(T k0, T k1, T w0, T w1, T x0, T x1) {
+    // pre-scaled doubled face flux (Table 2): (k0'+k1')(w1-w0) + (x0+x1), k' = the stored a' or c',
+    // x = b x (tangential difference of W) of the two cells the face separates (see StepCoef)
+    return fma_(add(k0, k1), sub(w1, w0), add(x0, x1));
 }
 // cross term b (W_+ - W_-) of one cell (G: y difference, H: x difference)
 template <typename T>

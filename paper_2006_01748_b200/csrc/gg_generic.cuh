@@ -22,9 +22,8 @@ struct GenericArgs {
     const T* __restrict__ a;   // [ny][nx]
     const T* __restrict__ b;
     const T* __restrict__ c;
-    const SimScalars* __restrict__ sims;  // [B]
+    const StepCoef<double>* __restrict__ coefs;  // [B], folded on the device (gg_dt.cuh)
     int nx, ny, nbatch;
-    double dt, dx, dy;
 };
 
 template <typename T>
@@ -38,7 +37,7 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T* U = A.U + sim * plane;
     const T* V = A.V + sim * plane;
     const T* W = A.W + sim * plane;
-    const StepCoef<T> k = fold_coef<T>(A.sims[sim], A.dt, A.dx, A.dy);
+    const StepCoef<T> k = load_coef<T>(A.coefs + sim);
 
     const bool hasW = i > 0, hasE = i < nx - 1, hasS = j > 0, hasN = j < ny - 1;
     const int iw = hasW ? i - 1 : i, ie = hasE ? i + 1 : i;
@@ -64,10 +63,10 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T HN = cross(at(A.b, i, jn), wNE, wNW);
     const T HS = cross(at(A.b, i, js), wSE, wSW);
     const T a0 = at(A.a, i, j), c0 = at(A.c, i, j);
-    T fE = flux_W(a0, at(A.a, ie, j), w, wE, G0, GE, k.thx);
-    T fW = flux_W(at(A.a, iw, j), a0, wW, w, GW, G0, k.thx);
-    T fN = flux_W(c0, at(A.c, i, jn), w, wN, H0, HN, k.thy);
-    T fS = flux_W(at(A.c, i, js), c0, wS, w, HS, H0, k.thy);
+    T fE = flux_W(a0, at(A.a, ie, j), w, wE, G0, GE);
+    T fW = flux_W(at(A.a, iw, j), a0, wW, w, GW, G0);
+    T fN = flux_W(c0, at(A.c, i, jn), w, wN, H0, HN);
+    T fS = flux_W(at(A.c, i, js), c0, wS, w, HS, H0);
     // zero total normal flux through boundary faces (the cross part does not vanish by clamping)
     if (!hasE) fE = (T)0;
     if (!hasW) fW = (T)0;

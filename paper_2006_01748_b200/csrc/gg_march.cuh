@@ -118,7 +118,7 @@ struct MarchWindow {
 #pragma unroll
         for (int f = 0; f <= C; ++f) {
             pV[f] = flux_V(uC[f], uC[f + 1], vC[f], vC[f + 1]);
-            pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1], k.thx);
+            pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1]);
         }
         if (atW) { pV[0] = (T)0; pW[0] = (T)0; }
         if (atE) { pV[C] = (T)0; pW[C] = (T)0; }
@@ -126,7 +126,7 @@ struct MarchWindow {
 #pragma unroll
         for (int c = 0; c < C; ++c) {
             nV[c] = flux_V(uC[c + 1], uN[c + 1], vC[c + 1], vN[c + 1]);
-            nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c], k.thy);
+            nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c]);
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {

@@ -36,12 +36,11 @@ struct alignas(64) PairArgs {
     void* U1;
     void* V1;
     void* W1;
-    const SimScalars* sims;
+    const StepCoef<double>* coefs;   // [B], folded on the device (gg_dt.cuh)
     int nx, ny, nbatch;
     int nw;                               // strips (compute warps) per CTA
     int ntilecols, nchunks, chunk_rows;
     long long nitems;
-    double dt, dx, dy;
 };
 
 template <typename T> __host__ __device__ constexpr int pair_gw() { return sizeof(T) == 8 ? 4 : 2; }
@@ -107,12 +106,12 @@ struct PairLevel {
             const T uW = shfl_up1(uC[C - 1]), vW = shfl_up1(vC[C - 1]), aW = shfl_up1(aC[C - 1]);
             const T wW = shfl_up1(wC[C - 1]), GW = shfl_up1(G[C - 1]);
             pV[0] = flux_V(uW, uC[0], vW, vC[0]);
-            pW[0] = flux_W(aW, aC[0], wW, wC[0], GW, G[0], k.thx);
+            pW[0] = flux_W(aW, aC[0], wW, wC[0], GW, G[0]);
         }
 #pragma unroll
         for (int f = 1; f < C; ++f) {
             pV[f] = flux_V(uC[f - 1], uC[f], vC[f - 1], vC[f]);
-            pW[f] = flux_W(aC[f - 1], aC[f], wC[f - 1], wC[f], G[f - 1], G[f], k.thx);
+            pW[f] = flux_W(aC[f - 1], aC[f], wC[f - 1], wC[f], G[f - 1], G[f]);
         }
         pV[C] = shfl_down1(pV[0]);
         pW[C] = shfl_down1(pW[0]);
@@ -122,7 +121,7 @@ struct PairLevel {
 #pragma unroll
         for (int c = 0; c < C; ++c) {
             nV[c] = flux_V(uC[c], uN[c], vC[c], vN[c]);
-            nW[c] = flux_W(cC[c], cN[c], wC[c], wN[c], hC[c], hN[c], k.thy);
+            nW[c] = flux_W(cC[c], cN[c], wC[c], wN[c], hC[c], hN[c]);
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {
@@ -249,7 +248,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_pair(const __grid_constant__ P
         const int iown = it.i0 + warp * VW + (lane - 1) * C;  // first own cell (lane 0: halo, may be < 0)
         const bool store_ok = lane_ok && iown < nx;
         const bool atW = iown == 0, atE = iown + C == nx;
-        const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+        const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
         T* gU = (T*)A.U1 + it.sim * plane + iown;
         T* gV = (T*)A.V1 + it.sim * plane + iown;
         T* gW = (T*)A.W1 + it.sim * plane + iown;

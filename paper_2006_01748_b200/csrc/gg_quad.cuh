@@ -22,6 +22,11 @@
 //    time-k+4 rows j0 .. j1-1.
 //  * Both roles run the SAME row body (PairLevel twice); they differ in where a row comes from and
 //    where the result goes.  Arithmetic and operand order are every other kernel's => bit-identical.
+//  * "C" builds (NSTC > 0, the fp64 default): the coefficient rows a, b, c do not change in time,
+//    so the B warps need not receive them from the A warps: their last-releasing warp fetches the
+//    B rows' own coefficient boxes by TMA (L2-hot: the A warps' TMA just read them) into a third
+//    ring.  ring1 then carries U, V, W only and the A warps shed three of their six shared-memory
+//    stores per row.  Needs one TMA box per array and row (fp64).
 #pragma once
 #include "gg_pair.cuh"
 
@@ -34,8 +39,13 @@ template <typename T> __host__ __device__ constexpr int quad_ring0_stage(int rb)
     return 6 * (4 / pair_gw<T>()) * pair_slab_bytes(rb, pair_box_bytes<T>());
 }
 __host__ __device__ constexpr int quad_ring1_stage(int rb) { return 6 * rb * kQuadRing1Runs * 16; }
-template <typename T> __host__ __device__ constexpr int quad_smem_bytes(int rb, int nst0, int nst1) {
-    return 256 + nst0 * quad_ring0_stage<T>(rb) + nst1 * quad_ring1_stage(rb);
+// nstc == 0: ring1 carries U, V, W and the rows' a, b, c.  nstc > 0 (the "C" builds, fp64): the
+// B warps fetch their own coefficient rows by TMA into a third ring of nstc stages and ring1
+// carries U, V, W only.
+template <typename T> __host__ __device__ constexpr int quad_smem_bytes(int rb, int nst0, int nst1, int nstc) {
+    return 256 + nst0 * quad_ring0_stage<T>(rb) +
+           (nstc > 0 ? nst1 * (quad_ring1_stage(rb) / 2) + nstc * (quad_ring0_stage<T>(rb) / 2)
+                     : nst1 * quad_ring1_stage(rb));
 }
 
 template <int RB>
@@ -47,8 +57,9 @@ __device__ __forceinline__ PairItem quad_item(const PairArgs& A, long long item,
 }
 
 // blockDim = 256: warps 0..3 = A, 4..7 = B.  Dynamic shared memory:
-// [full0[NST0], full1[NST1], empty1[NST1] mbarriers, count0[NST0]; 256 B][ring0][ring1].
-template <typename T, int RB, int NST0, int NST1>
+// [full0[NST0], full1[NST1], empty1[NST1], fullC[NSTC] mbarriers, count0[NST0], countC[NSTC];
+//  256 B][ring0: 6 arrays][ringC: a,b,c for the B warps (NSTC > 0)][ring1: U,V,W (+ a,b,c if NSTC == 0)].
+template <typename T, int RB, int NST0, int NST1, int NSTC>
 __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ PairArgs A) {
     constexpr int C = 16 / (int)sizeof(T);
     constexpr int GW = pair_gw<T>();
@@ -57,19 +68,26 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
     constexpr int BOXB = pair_box_bytes<T>();
     constexpr int SLAB = pair_slab_bytes(RB, BOXB);
     constexpr int ARR0 = NG * SLAB, STAGE0 = 6 * ARR0;
-    constexpr int P1 = kQuadRing1Runs * 16, ARR1 = RB * P1, STAGE1 = 6 * ARR1;
-    static_assert(STAGE0 == quad_ring0_stage<T>(RB) && STAGE1 == quad_ring1_stage(RB), "layout");
-    static_assert((NST0 + 2 * NST1) * 8 + NST0 * 4 <= 256, "too many stages");
+    constexpr bool CB = NSTC > 0;                       // B warps own a coefficient ring
+    constexpr int NF1 = CB ? 3 : 6;                     // arrays travelling through ring1
+    constexpr int P1 = kQuadRing1Runs * 16, ARR1 = RB * P1, STAGE1 = NF1 * ARR1;
+    constexpr int STAGEC = 3 * ARR0;
+    static_assert(STAGE0 == quad_ring0_stage<T>(RB), "layout");
+    static_assert(!CB || NG == 1, "the C builds need one TMA box per array and row (fp64)");
+    static_assert((NST0 + 2 * NST1 + NSTC) * 8 + (NST0 + NSTC) * 4 <= 256, "too many stages");
 
     extern __shared__ __align__(128) char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool isA = warp < 4;
     const int w = warp & 3;
     const uint32_t full0 = smem_u32(smem), full1 = full0 + 8u * NST0, empty1 = full1 + 8u * NST1;
-    unsigned int* count0 = reinterpret_cast<unsigned int*>(smem + 8 * (NST0 + 2 * NST1));
+    const uint32_t fullC = empty1 + 8u * NST1;
+    unsigned int* count0 = reinterpret_cast<unsigned int*>(smem + 8 * (NST0 + 2 * NST1 + NSTC));
+    unsigned int* countC = count0 + NST0;
     char* ring0 = smem + 256;
-    char* ring1 = ring0 + (size_t)NST0 * STAGE0;
-    const uint32_t ring0_u32 = smem_u32(ring0);
+    char* ringC = ring0 + (size_t)NST0 * STAGE0;      // TMA destinations first: 128-byte aligned
+    char* ring1 = ringC + (size_t)NSTC * STAGEC;
+    const uint32_t ring0_u32 = smem_u32(ring0), ringC_u32 = smem_u32(ringC);
     const int nx = A.nx, ny = A.ny;
     const int tile_cells = kQuadRuns * C;
     constexpr int NBOX = 6 * NG;
@@ -89,6 +107,19 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
                         f < 3 ? pc.it.sim : 0);
         }
     };
+    // C builds: the B warps' coefficient rows of the cursor's stage (a, b, c two rows below the A
+    // warps' rows)
+    auto issueC = [&](const PairCursor& pc, uint32_t slot) {
+        const uint32_t bar = fullC + 8u * slot;
+        const uint32_t dst = ringC_u32 + slot * STAGEC;
+        const int y = pc.it.j0 - 6 + pc.q * RB;
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(3 * RB * BOXB));
+        __syncwarp();
+        if (lane < 3) {
+            const CUtensorMap* map = lane == 0 ? &A.ma : lane == 1 ? &A.mb : &A.mc;
+            tma_load_3d(dst + lane * ARR0, map, bar, pc.it.i0 - 2 * C, y, 0);
+        }
+    };
     auto advance_cursor = [&](PairCursor& pc) {
         if (pc.item >= A.nitems) return;
         if (++pc.q == pc.it.nstage) {
@@ -100,6 +131,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NST0; ++s) { mbar_init(full0 + 8u * s, 1); count0[s] = 0u; }
+        for (int s = 0; s < NSTC; ++s) { mbar_init(fullC + 8u * s, 1); countC[s] = 0u; }
         for (int s = 0; s < NST1; ++s) { mbar_init(full1 + 8u * s, 4); mbar_init(empty1 + 8u * s, 4); }
         fence_barrier_init();
         fence_proxy_async();
@@ -118,12 +150,22 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
             if (warp == 0 && pc.item < A.nitems) issue(pc, (uint32_t)s);
             advance_cursor(pc);
         }
+    } else if constexpr (CB) {
+        for (int s = 0; s < NSTC; ++s) {
+            if (warp == 4 && pc.item < A.nitems) issueC(pc, (uint32_t)s);
+            advance_cursor(pc);
+        }
     }
 
     // where this lane finds its run in a stage of its source ring, and the ring's strides
     const int src_off = isA ? (w / GW) * SLAB + (w % GW) * (VW * (int)sizeof(T)) + 16 * lane
                             : (30 * w + lane + 1) * 16;
     const int src_arr = isA ? ARR0 : ARR1, src_row = isA ? BOXB : P1;
+    // coefficient rows: A finds them in its ring0 stage (arrays 3..5); B in ring1 (arrays 3..5) or,
+    // in the C builds, in its own box (same origin as ring0's boxes: run -2; the outermost lane of
+    // B warp 3 owns run 120, one past the box: it reads, and discards, the last run)
+    const int cof_off = isA || !CB ? src_off : min((30 * w + lane + 1) * 16, BOXB - 16);
+    const int cof_arr = isA || CB ? ARR0 : ARR1, cof_row = isA || CB ? BOXB : P1;
     const int dst_off = (30 * w + lane) * 16;              // A: own run in a ring1 row
     const int run0 = isA ? 30 * w - 2 + lane : 30 * w - 1 + lane;  // tile run this lane owns
     const bool lane_ok = lane >= 1 && lane <= (isA || w < 3 ? kPairLanes : kPairLanes - 2);
@@ -135,7 +177,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
         const int iown = it.i0 + run0 * C;               // first own cell (may lie outside the domain)
         const bool store_ok = lane_ok && iown >= 0 && iown < nx;
         const bool atW = iown == 0, atE = iown + C == nx;
-        const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+        const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
         T* gU = (T*)A.U1 + it.sim * plane + iown;
         T* gV = (T*)A.V1 + it.sim * plane + iown;
         T* gW = (T*)A.W1 + it.sim * plane + iown;
@@ -145,14 +187,17 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
         L2.clear();
 
         for (int q = 0; q < it.nstage; ++q, ++gc) {
-            const uint32_t s0 = gc % NST0, s1 = gc % NST1;
+            const uint32_t s0 = gc % NST0, s1 = gc % NST1, sc = CB ? gc % (CB ? NSTC : 1) : 0u;
             if (isA) {
                 mbar_wait(full0 + 8u * s0, (gc / NST0) & 1u);
                 if (gc >= NST1) mbar_wait(empty1 + 8u * s1, ((gc / NST1) - 1u) & 1u);
             } else {
+                if constexpr (CB) mbar_wait(fullC + 8u * sc, (gc / (CB ? NSTC : 1)) & 1u);
                 mbar_wait(full1 + 8u * s1, (gc / NST1) & 1u);
             }
             const char* src = (isA ? ring0 + (size_t)s0 * STAGE0 : ring1 + (size_t)s1 * STAGE1) + src_off;
+            const char* cof = (isA ? ring0 + (size_t)s0 * STAGE0 + 3 * ARR0
+                               : CB ? ringC + (size_t)sc * STAGEC : ring1 + (size_t)s1 * STAGE1 + 3 * ARR1) + cof_off;
             char* dst = ring1 + (size_t)s1 * STAGE1 + dst_off;
             // first row arriving at this role in this stage: time k for A, time k+2 for B
             const int jfirst = it.j0 - 4 + q * RB - (isA ? 0 : 2);
@@ -164,22 +209,25 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
                 ld_run<T, C>(p + 0 * src_arr, uN);
                 ld_run<T, C>(p + 1 * src_arr, vN);
                 ld_run<T, C>(p + 2 * src_arr, wN);
-                ld_run<T, C>(p + 3 * src_arr, aN);
-                ld_run<T, C>(p + 4 * src_arr, bN);
-                ld_run<T, C>(p + 5 * src_arr, cN);
+                const char* pcf = cof + rr * cof_row;
+                ld_run<T, C>(pcf + 0 * cof_arr, aN);
+                ld_run<T, C>(pcf + 1 * cof_arr, bN);
+                ld_run<T, C>(pcf + 2 * cof_arr, cN);
                 T u1[C], v1[C], w1[C], a1[C], b1[C], c1[C];   // row jn-1, one level up
                 L1.template advance<GHOST>(jn, ny, atW, atE, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
                 T u2[C], v2[C], w2[C], a2[C], b2[C], c2[C];   // row jn-2, two levels up
                 L2.template advance<GHOST>(jn - 1, ny, atW, atE, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
                 if (isA) {
-                    if (lane_ok) {                            // time-k+2 row jn-2 and its coefficients
+                    if (lane_ok) {                            // time-k+2 row jn-2 (and its coefficients)
                         char* o = dst + rr * P1;
                         st_run<T, C>(o + 0 * ARR1, u2);
                         st_run<T, C>(o + 1 * ARR1, v2);
                         st_run<T, C>(o + 2 * ARR1, w2);
-                        st_run<T, C>(o + 3 * ARR1, a2);
-                        st_run<T, C>(o + 4 * ARR1, b2);
-                        st_run<T, C>(o + 5 * ARR1, c2);
+                        if constexpr (!CB) {
+                            st_run<T, C>(o + 3 * ARR1, a2);
+                            st_run<T, C>(o + 4 * ARR1, b2);
+                            st_run<T, C>(o + 5 * ARR1, c2);
+                        }
                     }
                 } else {
                     const int r = jn - 2;                     // time-k+4 row
@@ -199,9 +247,10 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
                 for (int rr = 0; rr < RB; ++rr) row_body(std::true_type{}, rr);
             }
             __syncwarp();
+            // Slot hand-off.  A: ring1 stage written (release); ring0 slot read: the A warp that
+            // releases it last refills it with the stage NST0 ahead.  B: ring1 stage read; in the
+            // C builds the B warp that releases the coefficient slot last refills it.
             if (isA) {
-                // ring1 stage written (release); ring0 slot read: the A warp that releases it last
-                // refills it with the stage NST0 ahead
                 unsigned int prev = 0;
                 if (lane == 0) {
                     mbar_arrive(full1 + 8u * s1);
@@ -212,6 +261,19 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
                 if (prev == 3u) {
                     if (lane == 0) { count0[s0] = 0u; __threadfence_block(); }
                     if (pc.item < A.nitems) issue(pc, s0);
+                }
+                advance_cursor(pc);
+            } else if constexpr (CB) {
+                unsigned int prev = 0;
+                if (lane == 0) {
+                    mbar_arrive(empty1 + 8u * s1);
+                    __threadfence_block();
+                    prev = atomicAdd(&countC[sc], 1u);
+                }
+                prev = __shfl_sync(0xffffffffu, prev, 0);
+                if (prev == 3u) {
+                    if (lane == 0) { countC[sc] = 0u; __threadfence_block(); }
+                    if (pc.item < A.nitems) issueC(pc, sc);
                 }
                 advance_cursor(pc);
             } else if (lane == 0) {

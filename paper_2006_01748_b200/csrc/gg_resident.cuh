@@ -28,7 +28,7 @@ struct ResidentArgs {
     const void* U0; const void* V0; const void* W0;   // state at time k   [B][ny][nx]
     void* U1; void* V1; void* W1;                     // state at time k+n [B][ny][nx]
     const void* a; const void* b; const void* c;      // [ny][nx]
-    const SimScalars* sims;
+    const StepCoef<double>* coefs;   // [B], folded on the device (gg_dt.cuh)
     void* halo;                 // [2 parity][nslabs][2 sides][3 fields][nx] elements
     unsigned int* flags;        // [nslabs] last step whose edge rows the slab has published
     int nx, ny, nbatch;
@@ -36,7 +36,6 @@ struct ResidentArgs {
     int pitch;                  // shared-memory row pitch in bytes (nx * sizeof(T) + 32)
     long long nsteps;
     unsigned int epoch;         // flags start at epoch (set by the host before the launch)
-    double dt, dx, dy;
 };
 
 __host__ __device__ constexpr int resident_pitch(int nx, int esize) { return nx * esize + 32; }
@@ -76,7 +75,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_resident(const ResidentArgs A)
     const bool valid = iown < nx;
     const bool atW = iown == 0, atE = iown + C == nx;
     const size_t plane = (size_t)nx * ny;
-    const StepCoef<T> k = fold_coef<T>(A.sims[sim], A.dt, A.dx, A.dy);
+    const StepCoef<T> k = load_coef<T>(A.coefs + sim);
     const int own = 16 + 16 * t;   // byte offset of the lane's run inside a shared-memory row
 
     // ---- start-up: zero everything, then load the slab (+ halo rows inside the domain)

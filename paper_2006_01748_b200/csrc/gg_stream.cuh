@@ -49,11 +49,10 @@ struct alignas(64) StreamArgs {
     void* U1;                            // outputs [B][ny][nx]
     void* V1;
     void* W1;
-    const SimScalars* sims;
+    const StepCoef<double>* coefs;   // [B], folded on the device (gg_dt.cuh)
     int nx, ny, nbatch;
     int ntilecols, nchunks, chunk_rows;
     long long nitems;
-    double dt, dx, dy;
 };
 
 // Host-side plan: tensor maps for both ping-pong copies and the launch geometry.
@@ -246,7 +245,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) gg_step_stream(const __grid_
         const int iown = it.i0 + warp * SW + lane * C;  // first own cell
         const bool valid = iown < nx;                   // nx % C == 0: a run is all in or all out
         const bool atW = iown == 0, atE = iown + C == nx;
-        const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+        const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
         T* gU = (T*)A.U1 + it.sim * plane + iown;
         T* gV = (T*)A.V1 + it.sim * plane + iown;
         T* gW = (T*)A.W1 + it.sim * plane + iown;

@@ -168,7 +168,7 @@ gg_step_stream2(const __grid_constant__ StreamArgs A) {
         uint32_t g = 0;
         for (long long item = blockIdx.x; item < A.nitems; item += gridDim.x) {
             const Stream2Item it = stream2_item<RB, NW * SW>(A, item);
-            const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+            const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
             MarchWindow<T, 1> win;
             win.clear();
             for (int q = 0; q < it.nstage; ++q, ++g) {
@@ -215,7 +215,7 @@ gg_step_stream2(const __grid_constant__ StreamArgs A) {
             const Stream2Item it = stream2_item<RB, NW * SW>(A, item);
             const int iown = it.i0 + warp * SW + lane * C;
             const bool atW = iown == 0, atE = iown + C == nx;
-            const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+            const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
             MarchWindow<T, C> win;
             win.clear();
             for (int q = 0; q < it.nstage; ++q, ++g) {
@@ -266,7 +266,7 @@ gg_step_stream2(const __grid_constant__ StreamArgs A) {
             const int iown = it.i0 + w * SW + lane * C;
             const bool valid = iown < nx;
             const bool atW = iown == 0, atE = iown + C == nx;
-            const StepCoef<T> k = fold_coef<T>(A.sims[it.sim], A.dt, A.dx, A.dy);
+            const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
             T* gU = (T*)A.U1 + it.sim * plane + iown;
             T* gV = (T*)A.V1 + it.sim * plane + iown;
             T* gW = (T*)A.W1 + it.sim * plane + iown;

@@ -12,29 +12,36 @@ from paper_2006_01748_b200 import binding, build
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "gg.h")).read()
+def declared_symbols(header=os.path.join(ROOT, "include", "gg.h")):
+    src = open(header).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(gg_[a-z0-9_]+)\s*\(", src)))
+
+
+TUNING_H = os.path.join(ROOT, "paper_2006_01748_b200", "csrc", "gg_tuning.h")
 
 
 def test_header_declares_the_north_star_calls():
     names = declared_symbols()
     for need in ("gg_create", "gg_set_tensor", "gg_set_state", "gg_step", "gg_get_state"):
         assert need in names
+    # tuning knobs are not part of the installed interface
+    text = open(os.path.join(ROOT, "include", "gg.h")).read()
+    assert "_VARIANT" not in text and "gg_num_" not in text
 
 
 def test_library_builds_and_exports_every_declared_symbol():
     path = build.build()
     assert os.path.exists(path)
     lib = ctypes.CDLL(path)
-    for name in declared_symbols():
+    for name in declared_symbols() + declared_symbols(TUNING_H):
         assert hasattr(lib, name), f"libgg.so does not export {name}"
 
 
 def test_binding_covers_exactly_the_header():
     assert sorted(binding.SIGNATURES) == declared_symbols()
-    for name in binding.SIGNATURES:
+    assert sorted(binding.TUNING_SIGNATURES) == declared_symbols(TUNING_H)
+    for name in list(binding.SIGNATURES) + list(binding.TUNING_SIGNATURES):
         assert callable(getattr(binding, name)), f"binding lacks a function named {name}"
 
 

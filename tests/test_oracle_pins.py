@@ -517,3 +517,66 @@ def test_front_positions_brute_force_and_disk():
     wl = workloads.make(0)
     lo, hi = oracle.front(wl.V[0], 0, 32, 0.5)
     assert (lo, hi) == (26, 37) and oracle.front(wl.V[0], 1, 32, 0.5) == (26, 37)
+
+
+# ---------------------------------------------------------------------------------------------
+# Non-uniform step size dt_k (NEXT-2; the RULE is reading A6 and "parity unpinned": PAPER.md:62
+# prints no formula.  What is pinned here is its arithmetic and the time loop around it.)
+# ---------------------------------------------------------------------------------------------
+def test_adaptive_dt_worked_values_and_brute_force():
+    # worked value: A = diag(0.02, 0.01), b = 0 => lambda_max = 0.02; U = 0.75 everywhere and
+    # alpha = 0.2 => alpha (1 - U) = 0.05 > lambda_max; h = 0.5, safety = 0.1 => 0.1 * 0.25 / 0.05
+    a, b, c = np.full((3, 4), 0.02), np.zeros((3, 4)), np.full((3, 4), 0.01)
+    U = np.full((3, 4), 0.75)
+    assert oracle.adaptive_dt(U, a, b, c, 0.2, 0.5, safety=0.1) == pytest.approx(0.5, rel=1e-15)
+    # alpha (1 - U) below lambda_max: the tensor decides, 0.1 * 0.25 / 0.02
+    assert oracle.adaptive_dt(U, a, b, c, 0.04, 0.5, safety=0.1) == pytest.approx(1.25, rel=1e-15)
+    # dx != dy: the smaller mesh size enters squared
+    assert oracle.adaptive_dt(U, a, b, c, 0.2, 0.5, dy=0.25, safety=0.1) == pytest.approx(0.125, rel=1e-15)
+    # brute force on a random batch: max over simulations and cells written as loops
+    rng = np.random.default_rng(77)
+    Ub = rng.uniform(-0.1, 1.1, (3, 5, 6))      # includes U > 1 (1 - U < 0) and U < 0
+    al = np.array([0.03, 0.5, 0.2])
+    aa, bb, cc = rng.uniform(5e-3, 2e-2, (5, 6)), rng.uniform(-4e-3, 4e-3, (5, 6)), rng.uniform(5e-3, 2e-2, (5, 6))
+    rate = max(np.linalg.eigvalsh(np.array([[aa[j, i], bb[j, i]], [bb[j, i], cc[j, i]]]))[1]
+               for j in range(5) for i in range(6))
+    for s in range(3):
+        for j in range(5):
+            for i in range(6):
+                rate = max(rate, al[s] * (1.0 - Ub[s, j, i]))
+    assert oracle.adaptive_dt(Ub, aa, bb, cc, al, 0.25, safety=0.2) == pytest.approx(0.2 * 0.0625 / rate, rel=1e-14)
+    # where the V diffusivity sits at its bound alpha (some cell has U = 0) the rule IS reading
+    # A6's max_stable_dt
+    Ub[1, 2, 3] = 0.0
+    Ub = np.clip(Ub, 0.0, 1.0)
+    assert oracle.adaptive_dt(Ub, aa, bb, cc, al, 0.25, safety=0.2) == \
+        oracle.max_stable_dt(aa, bb, cc, al, 0.25, safety=0.2)
+
+
+def test_step_adaptive_is_the_step_with_hand_fed_step_sizes():
+    w = workloads.random_problem(61, 20, 14, batch=2)
+    al = np.array([0.2, 0.3])                        # alpha (1 - U) above lambda_max ~ 0.035: U drives dt_k
+    U0 = 0.6 + 0.4 * w.U                              # 1 - U starts in [0, 0.4] and grows as W kills U
+    kw = dict(r=w.r, d=w.d * 4.0, alpha=al, c_r=w.c_r)
+    U, V, W, t, dts = oracle.step_adaptive(U0, w.V, w.W, w.a, w.b, w.c, n=23, safety=0.2, every_k=5,
+                                           dx=w.h, **kw)
+    assert len(dts) == 5 and t == pytest.approx(sum(dts[:4]) * 5 + dts[4] * 3, rel=1e-15)
+    assert dts[0] > dts[-1] > 0                       # U decays => the V diffusivity bound grows
+    # replay by hand: the same groups through `step`, dt_k recomputed from the definition
+    Uh, Vh, Wh = U0.copy(), w.V.copy(), w.W.copy()
+    for g, n in enumerate((5, 5, 5, 5, 3)):
+        rate = max(oracle.lambda_max(w.a, w.b, w.c), max(al[s] * (1.0 - Uh[s]).max() for s in range(2)))
+        dt = 0.2 * w.h ** 2 / rate
+        assert dt == pytest.approx(dts[g], rel=1e-15)
+        for s in range(2):
+            Uh[s], Vh[s], Wh[s] = oracle.step(Uh[s], Vh[s], Wh[s], w.a, w.b, w.c, r=w.r[s], d=4.0 * w.d[s],
+                                              alpha=al[s], c_r=w.c_r[s], n=n, dt=dts[g], dx=w.h)
+    assert np.array_equal(U, Uh) and np.array_equal(V, Vh) and np.array_equal(W, Wh)
+    # alpha far below lambda_max: dt_k is constant and the run IS the fixed-step run, bit for bit
+    U2, V2, W2, t2, dts2 = oracle.step_adaptive(w.U[0], w.V[0], w.W[0], w.a, w.b, w.c, r=1.0, d=3.0,
+                                                alpha=1e-4, c_r=1.0, n=9, safety=0.2, every_k=2, dx=w.h)
+    dt = oracle.max_stable_dt(w.a, w.b, w.c, 1e-4, w.h, safety=0.2)
+    assert dts2 == [dt] * 5
+    ref = oracle.step(w.U[0], w.V[0], w.W[0], w.a, w.b, w.c, r=1.0, d=3.0, alpha=1e-4, c_r=1.0, n=9,
+                      dt=dt, dx=w.h)
+    assert all(np.array_equal(x, y) for x, y in zip((U2, V2, W2), ref))
