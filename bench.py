@@ -13,18 +13,28 @@ Prints ONE JSON line on stdout:
   e2e           the same metric through the C ABI with HOST (pinned) buffers: upload tensor and
                 state, K steps, download state, all inside the timed region
   roofline      compulsory bytes (72 B per cell-update in fp64) / measured launch time against the
-                measured HBM copy peak (MEASURED_PEAKS.json)
+                measured HBM copy peak (MEASURED_PEAKS.json); `traffic` (ncu DRAM bytes per launch)
+                and `alu.instr_per_cell_step` come from profiles/ncu_traffic.json and are null
+                unless that record was made for the kernel that ran AND for the csrc/ on disk
+  configs       the other BASELINE.json configs (3 in fp32, 2, 4, 1, 0) on rank 0 at N = 1: GLUPS,
+                us per step, the kernel AUTO resolved to, window parity against the oracle
   cpu_baseline  the CPU oracle, as it stands, on a bounded sample of the same workload
 N > 1 (torchrun): the path does not shard without a halo exchange that north_star excludes, so
 every rank runs an independent replica of the same workload ("replicas only", weak scaling);
 value = all ranks' cell-updates / max-over-ranks device time.
 `--impl reference` times the oracle (the reference arm of this tier) on rank 0 only.
+`--record-traffic RAW.csv` (no GPU needed) turns `ncu -i X.ncu-rep --page raw --csv` output into
+the profiles/ncu_traffic.json entries of the kernels it contains.
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import glob
+import hashlib
 import json
 import os
+import re
 import subprocess
 import sys
 import threading
@@ -40,6 +50,8 @@ METRIC = "cell-updates/s, explicit finite-volume step, fp64 8192^2 (BASELINE con
 UNIT = "GLUPS"
 BYTES_PER_CELL = {"f64": 72.0, "f32": 36.0}   # 3 fields read + 3 written + 3 coefficients read
 FALLBACK_HBM_GBS = 6650.0                      # /opt/skills/guides/B200_PROFILING.md
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+WORKLOAD3 = "BASELINE.json configs[3]: 8192x8192 {dtype}, 6-band discontinuous tensor, 3 tumour disks, h=1/64, d=10, alpha=1e-3"
 
 
 def log(*a):
@@ -54,13 +66,66 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(kernel, dtype):
-    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the step kernel at
-    8192^2 from the committed `ncu --set full` capture (profiles/ncu_traffic.json), or None."""
+def csrc_sha16() -> str:
+    """Hash of the kernel sources on disk: an ncu record made for other sources is stale."""
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2006_01748_b200", "csrc", "*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_record(kernel_name):
+    """The committed ncu record of `kernel_name` (per launch at 8192^2) if it was captured from
+    the csrc/ now on disk, else None -- never a stale constant."""
     try:
-        return float(json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))[f"{kernel}_{dtype}"])
+        rec = json.load(open(TRAFFIC_JSON))
+        if rec.get("csrc_sha16") != csrc_sha16():
+            return None
+        return rec["kernels"].get(kernel_name)
     except Exception:
         return None
+
+
+def record_traffic(raw_csv):
+    """profiles/ncu_traffic.json entries from an `ncu --page raw --csv` dump of 8192^2 launches."""
+    rows = list(csv.reader(open(raw_csv)))
+    hdr = rows[0]
+    col = {h: i for i, h in enumerate(hdr)}
+
+    def num(r, name):
+        return float(r[col[name]].replace(",", "")) if name in col and r[col[name]] else None
+    try:
+        rec = json.load(open(TRAFFIC_JSON))
+        if rec.get("csrc_sha16") != csrc_sha16():
+            rec = {}
+    except Exception:
+        rec = {}
+    rec = {"csrc_sha16": csrc_sha16(), "kernels": rec.get("kernels", {}),
+           "source": "per launch at 8192x8192, from `ncu --set full` captures turned into CSV with "
+                     "`ncu -i X.ncu-rep --page raw --csv` and recorded by `python bench.py "
+                     "--record-traffic X.csv`; valid only for the csrc/ whose hash is csrc_sha16"}
+    for r in rows[2:]:
+        name = re.sub(r"\s+", "", r[col["Kernel Name"]])
+        m = re.match(r"(?:void)?(?:gg::)?(gg_step_\w+<[^>]*>)", name)
+        if not m:
+            continue
+        name = m.group(1)
+        f64 = "<double" in name
+        steps = 4 if "quad" in name else 2 if ("pair" in name or "stream2" in name) else 1
+        rd, wr = num(r, "dram__bytes_read.sum"), num(r, "dram__bytes_write.sum")
+        unit_rd = rows[1][col["dram__bytes_read.sum"]]
+        scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(unit_rd, 1.0)
+        pipe = "smsp__inst_executed_pipe_fp64.sum" if f64 else "smsp__inst_executed_pipe_fma.sum"
+        inst = num(r, pipe)
+        entry = {"traffic_bytes_per_launch": (rd + wr) * scale, "steps_per_launch": steps,
+                 "gpu_time_us_under_ncu": num(r, "gpu__time_duration.sum")}
+        if inst is not None:
+            entry["pipe_instr_per_cell_step"] = inst * 32.0 / (8192.0 * 8192.0 * steps)
+            entry["pipe_metric"] = pipe
+        rec["kernels"][name] = entry
+        log(f"recorded {name}: {entry}")
+    json.dump(rec, open(TRAFFIC_JSON, "w"), indent=1)
 
 
 class ClockSampler:
@@ -122,50 +187,44 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------
 # CPU oracle leg (cpu_baseline / --impl reference): the oracle as it stands, bounded sample
 # ---------------------------------------------------------------------------------------------
-def oracle_sample(wl, rows=1024, steps=4):
-    """Time `steps` oracle steps on the first `rows` rows of the workload (full width, so the
-    memory access pattern per row is the workload's).  Returns (GLUPS, description, threads)."""
+SAMPLE_ROWS = 2048
+
+
+def oracle_sample(wl, steps, warmup=1, min_seconds=0.0, rows=SAMPLE_ROWS):
+    """Time blocks of `steps` oracle steps on the first `rows` rows of the workload (full width,
+    so the memory access pattern per row is the workload's), repeated until `min_seconds` have
+    passed.  Returns (GLUPS, description, threads, seconds per step)."""
     import oracle
     rows = min(rows, wl.ny)
     sl = slice(0, rows)
     U, V, W = wl.U[0, sl], wl.V[0, sl], wl.W[0, sl]
     a, b, c = wl.a[sl], wl.b[sl], wl.c[sl]
     kw = dict(r=wl.r[0], d=wl.d[0], alpha=wl.alpha[0], c_r=wl.c_r[0], dt=wl.dt, dx=wl.h)
-    oracle.step(U, V, W, a, b, c, n=1, **kw)  # warm-up (page faults, library load)
-    t0 = time.perf_counter()
-    oracle.step(U, V, W, a, b, c, n=steps, **kw)
-    t = time.perf_counter() - t0
-    glups = rows * wl.nx * steps / t / 1e9
-    desc = (f"oracle/gg_oracle.cpp (fp64, OpenMP over rows), {steps} steps on rows 0..{rows - 1} "
-            f"x all {wl.nx} columns of {wl.name}, {t:.2f} s")
-    return glups, desc, oracle.max_threads(), t
+    oracle.step(U, V, W, a, b, c, n=max(warmup, 1), **kw)  # warm-up (page faults, library load)
+    done, t = 0, 0.0
+    while done == 0 or t < min_seconds:
+        t0 = time.perf_counter()
+        oracle.step(U, V, W, a, b, c, n=steps, **kw)
+        t += time.perf_counter() - t0
+        done += steps
+    glups = rows * wl.nx * done / t / 1e9
+    desc = (f"oracle/gg_oracle.cpp (fp64, OpenMP over rows), {done} steps ({done // steps} x {steps}) on rows "
+            f"0..{rows - 1} x all {wl.nx} columns of {wl.name}, {t:.2f} s")
+    return glups, desc, oracle.max_threads(), t / done
 
 
 def run_reference(args, wl):
-    """Reference arm of this tier = the CPU oracle; K 'steps' are K oracle steps on the sample."""
-    import oracle
-    rows = 256                  # bounded: K steps at ~15 M cell-updates/s must end in minutes
-    sl = slice(0, rows)
-    U, V, W = wl.U[0, sl], wl.V[0, sl], wl.W[0, sl]
-    a, b, c = wl.a[sl], wl.b[sl], wl.c[sl]
-    kw = dict(r=wl.r[0], d=wl.d[0], alpha=wl.alpha[0], c_r=wl.c_r[0], dt=wl.dt, dx=wl.h)
-    K = min(args.steps, 400)
-    Wm = min(args.warmup, 3)
-    oracle.step(U, V, W, a, b, c, n=max(Wm, 1), **kw)
-    t0 = time.perf_counter()
-    oracle.step(U, V, W, a, b, c, n=K, **kw)
-    t = time.perf_counter() - t0
-    glups = rows * wl.nx * K / t / 1e9
-    sample = (f"{K} oracle steps on rows 0..{rows - 1} x all {wl.nx} columns of {wl.name} "
-              f"(bounded sample of the 8192^2 workload)")
+    """Reference arm of this tier = the CPU oracle.  A 'step' is one oracle step on the bounded
+    sample (rows 0..2047 x all columns of the 8192^2 workload); W warm-up steps, then blocks of K
+    timed steps until at least 2 s have passed."""
+    glups, desc, cores, s_per_step = oracle_sample(wl, args.steps, warmup=args.warmup, min_seconds=2.0)
     return {
         "impl": "reference", "metric": METRIC, "value": glups, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": K, "warmup": Wm, "ms_per_step": t / K * 1e3, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "BASELINE.json configs[3]: 8192x8192 fp64 layered tensor, 3 disks",
-                   "sample": sample},
-        "cpu_baseline": {"value": glups, "unit": UNIT, "cores": oracle.max_threads(),
-                         "kind": "oracle", "sample": sample},
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": s_per_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": WORKLOAD3.format(dtype="f64"), "sample": desc},
+        "cpu_baseline": {"value": glups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": glups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -195,6 +254,9 @@ def job_glups(cells_per_rank, steps, ms_local, world, device):
 # ---------------------------------------------------------------------------------------------
 # GPU leg
 # ---------------------------------------------------------------------------------------------
+KERNEL_IDS = ("generic", "stream", "stream2", "pair", "quad")
+
+
 def run_ours(args, wl, rank, world, device):
     import torch
     from paper_2006_01748_b200 import binding
@@ -215,12 +277,9 @@ def run_ours(args, wl, rank, world, device):
     sim = binding.Simulation(wl.nx, wl.ny, wl.h, wl.r, wl.d, wl.alpha, wl.c_r, dtype=dtype,
                              batch=wl.batch, device=str(device))
     if args.kernel:
-        sim.set_option(binding.GG_OPT_KERNEL, {"generic": binding.GG_KERNEL_GENERIC,
-                                               "stream": binding.GG_KERNEL_STREAM,
-                                               "stream2": binding.GG_KERNEL_STREAM2,
-                                               "pair": binding.GG_KERNEL_PAIR,
-                                               "quad": binding.GG_KERNEL_QUAD}[args.kernel])
-    for o, v in (("warps", binding.GG_OPT_STREAM_WARPS), ("variant", binding.GG_OPT_PAIR_VARIANT)):
+        sim.set_option(binding.GG_OPT_KERNEL, getattr(binding, "GG_KERNEL_" + args.kernel.upper()))
+    for o, v in (("warps", binding.GG_OPT_STREAM_WARPS), ("variant", binding.GG_OPT_PAIR_VARIANT),
+                 ("quad_variant", binding.GG_OPT_QUAD_VARIANT)):
         if getattr(args, o) is not None:
             sim.set_option(v, getattr(args, o))
     # pinned host copies of the inputs (what a host-side caller holds)
@@ -234,7 +293,6 @@ def run_ours(args, wl, rank, world, device):
     # ---- device-resident timing: W warm-up steps, then exactly K steps -----------------------
     sim.step(Wm, wl.dt)
     sim.step(K, wl.dt)          # builds and caches the K-step graphs (untimed)
-    binding.gg_set_state_host(sim.ctx, ptr(host["U"]), ptr(host["V"]), ptr(host["W"]))
     # enough repetitions of the K timed steps for nvidia-smi (100 ms period) to see the load
     est_ms = max(sim.last_step_ms(), 1e-3)
     nreps = max(args.reps, int(np.ceil(600.0 / est_ms)) if est_ms < 600.0 else args.reps)
@@ -271,14 +329,13 @@ def run_ours(args, wl, rank, world, device):
                    f"pinned host buffers, {h2d / 1e9:.2f} GB up and {d2h / 1e9:.2f} GB down per job",
            "seconds": e2e_s}
     final = tuple(out[k].numpy() for k in ("U", "V", "W"))
-    kernel = sim.kernel
+    kernel, kernel_name = sim.kernel, sim.kernel_name
     reductions = None
     if args.extras:
         # the device-side reductions next to the step: one pass over
-        # U, V, W resp. a, b, c = 3 arrays read; wall clock around the synchronising C-ABI call
-        # (includes the launch and the 8..64-byte result copy), median of 7
-        es = 8 if dtype == "f64" else 4
-
+        # U, V, W; wall clock around the synchronising C-ABI call (includes the launch and the
+        # result copy), median of 7.  And the adaptive step loop: dt_k re-evaluated on the device
+        # every 4 steps (one four-step launch per dt_k), against the fixed-dt loop above.
         def timed(fn):
             ts = []
             for _ in range(7):
@@ -288,41 +345,76 @@ def run_ours(args, wl, rank, world, device):
                 ts.append(time.perf_counter() - t0)
             return float(np.median(ts))
         t_diag = timed(lambda: sim.diagnostics(1e-2))
-        t_dt = timed(lambda: sim.max_stable_dt(0.2))
+        sim.step_adaptive(K, 0.2, 4)
+        ad = []
+        for _ in range(5):
+            sim.step_adaptive(K, 0.2, 4)
+            ad.append(sim.last_step_ms())
         reductions = {"gg_diagnostics_ms": t_diag * 1e3, "gg_diagnostics_gbs": 3 * cells * es / t_diag / 1e9,
-                      "gg_max_stable_dt_ms": t_dt * 1e3,
-                      "gg_max_stable_dt_gbs": 3 * wl.nx * wl.ny * es / t_dt / 1e9,
-                      "bound": "hbm", "bytes": "3 arrays read once, 24 B (fp64) / 12 B (fp32) per cell"}
+                      "bound": "hbm", "bytes": "3 arrays read once, 24 B (fp64) / 12 B (fp32) per cell",
+                      "gg_step_adaptive_every_4_glups": cells * K / (float(np.median(ad)) * 1e-3) / 1e9}
     sim.close()
     return dict(value=value, ms=ms / K, reps_ms=reps, launches=launches, e2e=e2e,
-                clocks=clk.summary(), kernel=kernel, final=final, reductions=reductions)
+                clocks=clk.summary(), kernel=kernel, kernel_name=kernel_name, final=final,
+                reductions=reductions)
 
 
-def sampled_parity(wl, final, K, size=48):
-    """Oracle check of the e2e end state on two windows the oracle can afford: the domain corner
-    (true Neumann faces on two sides) and a window on the rim of the first tumour disk.  A window
-    is cut with a margin of K cells on its interior sides (the stencil moves information one cell
-    per step), the oracle runs K steps on the cut, and only the uncontaminated core is compared."""
+def window_parity(wl, final, K, s=0, size=48):
+    """Oracle check of an end state on two windows the oracle can afford: the domain corner (true
+    Neumann faces on two sides) and a window on the rim of the first tumour disk.  A window is cut
+    with a margin of K cells on its interior sides (the stencil moves information one cell per
+    step), the oracle runs K steps on the cut, and only the uncontaminated core is compared."""
     import oracle
-    x, y = np.meshgrid(np.arange(wl.nx), np.arange(wl.ny), indexing="xy")
-    inside = wl.V[0] > 0.5
+    inside = wl.V[s] > 0.5
     jj, ii = np.nonzero(inside)
     k = np.argmin(ii)  # leftmost cell of a disk: a front
-    spots = {"corner": (0, 0), "front": (max(int(ii[k]) - size // 2, 0), max(int(jj[k]) - size // 2, 0))}
-    del x, y
+    size = min(size, wl.nx, wl.ny)
+    spots = {"corner": (0, 0), "front": (min(max(int(ii[k]) - size // 2, 0), wl.nx - size),
+                                          min(max(int(jj[k]) - size // 2, 0), wl.ny - size))}
     worst = 0.0
     for name, (i0, j0) in spots.items():
         ia, ja = max(i0 - K, 0), max(j0 - K, 0)
         ib, jb = min(i0 + size + K, wl.nx), min(j0 + size + K, wl.ny)
         cut = (slice(ja, jb), slice(ia, ib))
-        ref = oracle.step(wl.U[0][cut], wl.V[0][cut], wl.W[0][cut], wl.a[cut], wl.b[cut], wl.c[cut],
-                          r=wl.r[0], d=wl.d[0], alpha=wl.alpha[0], c_r=wl.c_r[0], n=K, dt=wl.dt,
+        ref = oracle.step(wl.U[s][cut], wl.V[s][cut], wl.W[s][cut], wl.a[cut], wl.b[cut], wl.c[cut],
+                          r=wl.r[s], d=wl.d[s], alpha=wl.alpha[s], c_r=wl.c_r[s], n=K, dt=wl.dt,
                           dx=wl.h)
         core = (slice(j0 - ja, j0 - ja + size), slice(i0 - ia, i0 - ia + size))
         full = (slice(j0, j0 + size), slice(i0, i0 + size))
         for f in range(3):
-            worst = max(worst, float(np.max(np.abs(final[f][0][full].astype(np.float64) - ref[f][core]))))
+            worst = max(worst, float(np.max(np.abs(final[f][s][full].astype(np.float64) - ref[f][core]))))
     return worst
+
+
+def other_configs(device, wl3):
+    """The other BASELINE.json configs with AUTO kernel selection, inputs resident in HBM: median
+    device time of 5 repetitions of K steps (K scaled to the config), and window parity of the end
+    state of ONE K-step run against the oracle.  Builder-side numbers become driver-side ones."""
+    import torch
+    from paper_2006_01748_b200 import binding, workloads
+    out = {}
+    plan = [("cfg3_f32", lambda: wl3, "f32", 40), ("cfg2_d10", lambda: workloads.make(2, d=10.0), "f64", 200),
+            ("cfg4_batch64", lambda: workloads.make(4), "f64", 40), ("cfg1", lambda: workloads.make(1), "f64", 400),
+            ("cfg0", lambda: workloads.make(0), "f64", 200)]
+    for name, mk, dtype, K in plan:
+        wl = mk()
+        with binding.from_workload(wl, dtype=dtype, device=str(device)) as sim:
+            sim.step(K, wl.dt)
+            final = sim.get_state_numpy()
+            err = max(window_parity(wl, final, K, s) for s in sorted({0, wl.batch - 1}))
+            ms = []
+            for _ in range(5):
+                sim.step(K, wl.dt)
+                ms.append(sim.last_step_ms())
+            torch.cuda.synchronize(device)
+            t = float(np.median(ms))
+            out[name] = {"workload": wl.name, "dtype": dtype, "steps": K, "kernel": sim.kernel,
+                         "kernel_name": sim.kernel_name, "glups": wl.cells * K / (t * 1e-3) / 1e9,
+                         "us_per_step": t * 1e3 / K, "parity_window_max_abs_err": err,
+                         "tolerance": 1e-10 if dtype == "f64" else 2e-4}
+        log(f"config {name}: {out[name]}")
+        del wl
+    return out
 
 
 def main():
@@ -332,15 +424,22 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--kernel", default=None, choices=[None, "generic", "stream", "stream2", "pair", "quad"])
+    ap.add_argument("--kernel", default=None, choices=[None, *KERNEL_IDS])
     ap.add_argument("--warps", type=int, default=None, help="tuning: GG_OPT_STREAM_WARPS")
     ap.add_argument("--variant", type=int, default=None, help="tuning: GG_OPT_PAIR_VARIANT")
+    ap.add_argument("--quad-variant", dest="quad_variant", type=int, default=None, help="tuning: GG_OPT_QUAD_VARIANT")
     ap.add_argument("--reps", type=int, default=3)
     ap.add_argument("--n", type=int, default=8192, help="grid edge (8192 = the headline config)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-configs", action="store_true", help="skip the `configs` object (other BASELINE configs)")
     ap.add_argument("--extras", action="store_true",
-                    help="also time gg_diagnostics / gg_max_stable_dt (adds a `reductions` object)")
+                    help="also time gg_diagnostics / gg_step_adaptive (adds a `reductions` object)")
+    ap.add_argument("--record-traffic", default=None, metavar="RAW.csv",
+                    help="update profiles/ncu_traffic.json from an `ncu --page raw --csv` dump and exit")
     args = ap.parse_args()
+    if args.record_traffic:
+        record_traffic(args.record_traffic)
+        return 0
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -372,23 +471,25 @@ def main():
         cells = wl.nx * wl.ny
         bpc = BYTES_PER_CELL[args.dtype]
         # roofline of the dominant (only) kernel: ALGORITHMIC bytes one launch accounts for
-        # (72 B x cells x time steps the launch advances) / its average duration.  The two-step
-        # kernel advances two steps per pass over HBM, so this may exceed the copy peak; `traffic`
-        # is what ncu saw the launch really move.
+        # (72 B x cells x time steps the launch advances) / its average duration.  A k-step
+        # kernel advances k steps per pass over HBM, so this may exceed the copy peak; `traffic`
+        # is what ncu saw the launch really move, frac_dram_actual the PHYSICAL fraction.
         launches = max(res["launches"], 1)
         steps_per_launch = args.steps / launches
         bytes_per_launch = cells * bpc * steps_per_launch
         launch_ms = res["ms"] * args.steps / launches
         achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
-        traffic = ncu_traffic(res["kernel"], args.dtype) if wl.nx == 8192 else None
+        rec = ncu_record(res["kernel_name"]) if wl.nx == 8192 else None
+        traffic = rec["traffic_bytes_per_launch"] if rec else None
+        dram_actual = (traffic / (launch_ms * 1e-3) / 1e9) if traffic else None
         line = {
             "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": res["ms"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": args.dtype, "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[3]: {wl.nx}x{wl.ny} {args.dtype}, 6-band "
-                                   "discontinuous tensor, 3 tumour disks, h=1/64, d=10, alpha=1e-3",
-                       "kernel": res["kernel"], "l2": "working set 4.8 GB per step >> 126 MB L2",
+            "config": {"workload": WORKLOAD3.format(dtype=args.dtype).replace("8192x8192", f"{wl.nx}x{wl.ny}"),
+                       "kernel": res["kernel"], "kernel_name": res["kernel_name"],
+                       "l2": "working set 4.8 GB per step >> 126 MB L2",
                        "multi_gpu": "replicas only" if world > 1 else "single GPU",
                        "timing": f"median of {len(res['reps_ms'])} repetitions of the {args.steps} timed steps "
                                  f"(min {min(res['reps_ms']):.3f} ms, max {max(res['reps_ms']):.3f} ms)"},
@@ -396,31 +497,37 @@ def main():
                          "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": bytes_per_launch,
                          "steps_per_launch": steps_per_launch, "launch_ms": launch_ms,
-                         "dram_gbs_actual": (traffic / (launch_ms * 1e-3) / 1e9) if traffic else None,
+                         "dram_gbs_actual": dram_actual,
+                         "frac_dram_actual": (dram_actual / peak) if dram_actual else None,
+                         "traffic_source": ("profiles/ncu_traffic.json, csrc " + csrc_sha16()) if rec else
+                                           "null: no ncu record for this kernel and this csrc/ (hash " + csrc_sha16() + ")",
                          "frac_of_nominal_8000": achieved / 8000.0},
             "e2e": res["e2e"], "gpu_launches": res["launches"], "clocks": res["clocks"],
         }
-        # The multi-step kernels are no longer HBM-bound (ncu: DRAM 3.8 TB/s for `quad`); their
-        # nearest ceiling is the plain-ALU pipe of the arithmetic type.  Thread instructions per
-        # cell-step from the ncu captures (fp64 / fp32 pipe instructions x 32 / cell-steps of the
-        # launch, redundant overlap lanes included); peak = 148 SMs x lanes per clock x the max SM
-        # clock (one fused multiply-add = one instruction), DESIGN.md section 8.
-        ops = {"quad": 43.0, "pair": 42.5, "stream2": 52.0, "stream": 52.0}.get(res["kernel"])
-        if ops is not None:
+        # The multi-step kernels are not HBM-bound (see frac_dram_actual); their nearest ceiling
+        # is the plain-ALU pipe of the arithmetic type.  Thread instructions of that pipe per
+        # cell-step from the ncu record of THIS kernel (redundant overlap lanes included); peak =
+        # 148 SMs x lanes per clock x the max SM clock (one fused multiply-add = one instruction),
+        # DESIGN.md section 8.  Absent when there is no valid record.
+        if rec and rec.get("pipe_instr_per_cell_step"):
+            ops = rec["pipe_instr_per_cell_step"]
             lanes = 64 if args.dtype == "f64" else 128
             mhz = (res["clocks"] or {}).get("sm_max_mhz") or 1965.0
             alu_peak = 148 * lanes * mhz * 1e6 / 1e12
             alu = res["value"] * 1e9 * ops / 1e12
             line["alu"] = {"bound": "alu", "achieved": alu, "peak": alu_peak,
                            "unit": f"T {args.dtype} instr/s", "frac": alu / alu_peak,
-                           "instr_per_cell_step": ops}
+                           "instr_per_cell_step": ops, "source": rec.get("pipe_metric")}
         if res.get("reductions"):
             line["reductions"] = res["reductions"]
         t0 = time.perf_counter()
-        line["parity_sample_max_abs_err"] = sampled_parity(wl, res["final"], args.steps)
+        line["parity_sample_max_abs_err"] = window_parity(wl, res["final"], args.steps)
         log(f"sampled parity: {line['parity_sample_max_abs_err']:.3e} ({time.perf_counter() - t0:.1f} s)")
+        res["final"] = None
+        if world == 1 and not args.no_configs and args.dtype == "f64" and not args.kernel and wl.nx == 8192:
+            line["configs"] = other_configs(device, wl)
         if not args.no_cpu and world == 1:
-            g, desc, cores, _ = oracle_sample(wl, rows=2048, steps=200)
+            g, desc, cores, _ = oracle_sample(wl, steps=50, min_seconds=6.0)
             line["cpu_baseline"] = {"value": g, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": desc}
         print(json.dumps(line), flush=True)

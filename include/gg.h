@@ -206,6 +206,9 @@ int gg_set_option(gg_ctx* ctx, int option, long long value);
  *                 recorded on the bound stream around its launches; synchronises on the end
  *                 event.  *ms < 0 if no step has run. */
 int gg_kernel_used(const gg_ctx* ctx);
+/* Name of the kernel instantiation behind gg_kernel_used, as a profiler prints it, e.g.
+ * "gg_step_quad<double,4,2,2,2>" (context-owned; "" before the first gg_step built its plan). */
+const char* gg_kernel_name(const gg_ctx* ctx);
 long long gg_launches(const gg_ctx* ctx);
 long long gg_graph_captures(const gg_ctx* ctx);
 int gg_last_step_ms(gg_ctx* ctx, float* ms);

@@ -59,6 +59,7 @@ SIGNATURES = {
                                 ctypes.POINTER(ctypes.c_int)]),
     "gg_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_longlong]),
     "gg_kernel_used": (ctypes.c_int, [_vp]),
+    "gg_kernel_name": (ctypes.c_char_p, [_vp]),
     "gg_launches": (ctypes.c_longlong, [_vp]),
     "gg_graph_captures": (ctypes.c_longlong, [_vp]),
     "gg_last_step_ms": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_float)]),
@@ -214,6 +215,10 @@ def gg_kernel_used(ctx) -> int:
     return int(load().gg_kernel_used(ctx))
 
 
+def gg_kernel_name(ctx) -> str:
+    return (load().gg_kernel_name(ctx) or b"").decode()
+
+
 def gg_launches(ctx) -> int:
     return int(load().gg_launches(ctx))
 
@@ -364,6 +369,10 @@ class Simulation:
     @property
     def kernel(self) -> str:
         return KERNEL_NAMES.get(gg_kernel_used(self.ctx), "?")
+
+    @property
+    def kernel_name(self) -> str:
+        return gg_kernel_name(self.ctx)
 
     @property
     def launches(self) -> int:

@@ -81,7 +81,7 @@ struct gg_ctx {
     // register-chained two-step kernel (gg_pair.cuh)
     struct PairPlan {
         CUtensorMap state[2][3], coef[3];
-        int nw = 0, ntilecols = 0, nchunks = 0, chunk_rows = 0, grid = 0, block = 0, rb = 0, nst = 0;
+        int nw = 0, ntilecols = 0, nchunks = 0, chunk_rows = 0, grid = 0, block = 0, rb = 0, nst = 0, nst1 = 0, nstc = 0;
         long long nitems = 0;
         size_t smem = 0;
         const void* fn = nullptr;
@@ -105,7 +105,7 @@ struct gg_ctx {
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool timed = false;
     int num_sms = 0;
-    mutable std::string err;
+    mutable std::string err, kname;
 
     size_t esize() const { return dtype == GG_F64 ? 8 : 4; }
     size_t plane() const { return (size_t)nx * ny; }
@@ -1008,6 +1008,35 @@ int gg_max_stable_dt(gg_ctx* ctx, double safety, double* dt, double* lambda_max)
 }
 
 int gg_kernel_used(const gg_ctx* ctx) { return ctx ? resolve_kernel(ctx) : -1; }
+
+const char* gg_kernel_name(const gg_ctx* ctx) {
+    if (!ctx) return "";
+    const char* T = ctx->dtype == GG_F64 ? "double" : "float";
+    char buf[128];
+    try {
+        switch (resolve_kernel(ctx)) {
+            case GG_KERNEL_GENERIC: snprintf(buf, sizeof buf, "gg_step_generic<%s>", T); break;
+            case GG_KERNEL_RESIDENT: snprintf(buf, sizeof buf, "gg_step_resident<%s>", T); break;
+            case GG_KERNEL_STREAM:
+                if (!ctx->plan_ready) return "";
+                snprintf(buf, sizeof buf, "gg_step_stream<%s,%d,%d,%d>", T, ctx->plan.rb, ctx->plan.nst, ctx->plan.nw); break;
+            case GG_KERNEL_STREAM2:
+                if (!ctx->plan2_ready) return "";
+                snprintf(buf, sizeof buf, "gg_step_stream2<%s,%d,%d,%d,%d>", T, ctx->plan2.rb, ctx->plan2.nst, ctx->plan2.nst1, ctx->plan2.nw); break;
+            case GG_KERNEL_PAIR:
+                if (!ctx->pair.ready) return "";
+                snprintf(buf, sizeof buf, "gg_step_pair<%s,%d,%d>", T, ctx->pair.rb, ctx->pair.nst); break;
+            case GG_KERNEL_QUAD:
+                if (!ctx->quad.ready) return "";
+                snprintf(buf, sizeof buf, "gg_step_quad<%s,%d,%d,%d,%d,%d>", T, ctx->quad.rb, ctx->quad.nst, ctx->quad.nst1, ctx->quad.nstc, ctx->quad.nw); break;
+            default: return "";
+        }
+        ctx->kname = buf;
+    } catch (...) {
+        return "";
+    }
+    return ctx->kname.c_str();
+}
 long long gg_launches(const gg_ctx* ctx) { return ctx ? ctx->launches : 0; }
 long long gg_graph_captures(const gg_ctx* ctx) { return ctx ? ctx->graph_captures : 0; }
 

@@ -134,9 +134,12 @@ gg_lambda_max_partial(const T* __restrict__ a, const T* __restrict__ b, const T*
     const size_t lo = (size_t)blockIdx.x * seg;
     const size_t hi = lo + seg < plane ? lo + seg : plane;
     double m = -INFINITY;
+    // rounding points written out (no FMA contraction): the value is a pure function of the
+    // stored entries, bit-identical to the same formula evaluated in plain fp64 anywhere
     auto lam = [](double aa, double bb, double cc) {
-        const double hd = 0.5 * (aa - cc);
-        return 0.5 * (aa + cc) + sqrt(hd * hd + bb * bb);
+        const double hd = __dmul_rn(0.5, __dsub_rn(aa, cc));
+        return __dadd_rn(__dmul_rn(0.5, __dadd_rn(aa, cc)),
+                         __dsqrt_rn(__dadd_rn(__dmul_rn(hd, hd), __dmul_rn(bb, bb))));
     };
     constexpr int VC = 16 / (int)sizeof(T);
     constexpr int UN = 4;

@@ -32,20 +32,26 @@
 
 namespace gg {
 
-constexpr int kQuadRuns = 118;         // output runs per tile row
-constexpr int kQuadRing1Runs = 123;    // runs per ring1 row (run -2 .. 120)
-
-template <typename T> __host__ __device__ constexpr int quad_ring0_stage(int rb) {
-    return 6 * (4 / pair_gw<T>()) * pair_slab_bytes(rb, pair_box_bytes<T>());
+// NWR = warps per role (A and B): 4 (one 8-warp CTA per SM), 3 (two 6-warp CTAs per SM) or 2 (three
+// 4-warp CTAs per SM).  Narrower tiles leave registers and shared memory for more warps per SM and
+// fit grid widths that 236-cell tiles pad badly (1024 cells = 4.34 tiles of 4 warps, 5.8 of 3).
+__host__ __device__ constexpr int quad_runs(int nwr) { return 30 * nwr - 2; }        // output runs per tile row
+__host__ __device__ constexpr int quad_ring1_runs(int nwr) { return 30 * nwr + 3; }  // runs per ring1 row (run -2 ..)
+template <typename T> __host__ __device__ constexpr int quad_gw(int nwr) { return nwr < pair_gw<T>() ? nwr : pair_gw<T>(); }
+// bytes of one TMA box row: up to GW strips of 30 runs plus one run of overlap on each side
+template <typename T> __host__ __device__ constexpr int quad_box_bytes(int nwr) { return quad_gw<T>(nwr) * kPairLanes * 16 + 32; }
+template <typename T> __host__ __device__ constexpr int quad_ng(int nwr) { return (nwr + quad_gw<T>(nwr) - 1) / quad_gw<T>(nwr); }
+template <typename T> __host__ __device__ constexpr int quad_ring0_stage(int rb, int nwr) {
+    return 6 * quad_ng<T>(nwr) * pair_slab_bytes(rb, quad_box_bytes<T>(nwr));
 }
-__host__ __device__ constexpr int quad_ring1_stage(int rb) { return 6 * rb * kQuadRing1Runs * 16; }
+__host__ __device__ constexpr int quad_ring1_stage(int rb, int nwr) { return 6 * rb * quad_ring1_runs(nwr) * 16; }
 // nstc == 0: ring1 carries U, V, W and the rows' a, b, c.  nstc > 0 (the "C" builds, fp64): the
 // B warps fetch their own coefficient rows by TMA into a third ring of nstc stages and ring1
 // carries U, V, W only.
-template <typename T> __host__ __device__ constexpr int quad_smem_bytes(int rb, int nst0, int nst1, int nstc) {
-    return 256 + nst0 * quad_ring0_stage<T>(rb) +
-           (nstc > 0 ? nst1 * (quad_ring1_stage(rb) / 2) + nstc * (quad_ring0_stage<T>(rb) / 2)
-                     : nst1 * quad_ring1_stage(rb));
+template <typename T> __host__ __device__ constexpr int quad_smem_bytes(int rb, int nst0, int nst1, int nstc, int nwr) {
+    return 256 + nst0 * quad_ring0_stage<T>(rb, nwr) +
+           (nstc > 0 ? nst1 * (quad_ring1_stage(rb, nwr) / 2) + nstc * (quad_ring0_stage<T>(rb, nwr) / 2)
+                     : nst1 * quad_ring1_stage(rb, nwr));
 }
 
 template <int RB>
@@ -56,30 +62,31 @@ __device__ __forceinline__ PairItem quad_item(const PairArgs& A, long long item,
     return it;
 }
 
-// blockDim = 256: warps 0..3 = A, 4..7 = B.  Dynamic shared memory:
+// blockDim = 64 NWR: warps 0..NWR-1 = A, NWR..2NWR-1 = B.  Dynamic shared memory:
 // [full0[NST0], full1[NST1], empty1[NST1], fullC[NSTC] mbarriers, count0[NST0], countC[NSTC];
 //  256 B][ring0: 6 arrays][ringC: a,b,c for the B warps (NSTC > 0)][ring1: U,V,W (+ a,b,c if NSTC == 0)].
-template <typename T, int RB, int NST0, int NST1, int NSTC>
-__global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ PairArgs A) {
+template <typename T, int RB, int NST0, int NST1, int NSTC, int NWR>
+__global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : NWR == 3 ? 2 : 3) gg_step_quad(const __grid_constant__ PairArgs A) {
     constexpr int C = 16 / (int)sizeof(T);
-    constexpr int GW = pair_gw<T>();
-    constexpr int NG = 4 / GW;
+    constexpr int GW = quad_gw<T>(NWR);
+    constexpr int NG = quad_ng<T>(NWR);
     constexpr int VW = kPairLanes * C;
-    constexpr int BOXB = pair_box_bytes<T>();
+    constexpr int BOXB = quad_box_bytes<T>(NWR);
     constexpr int SLAB = pair_slab_bytes(RB, BOXB);
     constexpr int ARR0 = NG * SLAB, STAGE0 = 6 * ARR0;
     constexpr bool CB = NSTC > 0;                       // B warps own a coefficient ring
     constexpr int NF1 = CB ? 3 : 6;                     // arrays travelling through ring1
-    constexpr int P1 = kQuadRing1Runs * 16, ARR1 = RB * P1, STAGE1 = NF1 * ARR1;
+    constexpr int P1 = quad_ring1_runs(NWR) * 16, ARR1 = RB * P1, STAGE1 = NF1 * ARR1;
     constexpr int STAGEC = 3 * ARR0;
-    static_assert(STAGE0 == quad_ring0_stage<T>(RB), "layout");
+    constexpr int NTHR = 64 * NWR;
+    static_assert(STAGE0 == quad_ring0_stage<T>(RB, NWR), "layout");
     static_assert(!CB || NG == 1, "the C builds need one TMA box per array and row (fp64)");
     static_assert((NST0 + 2 * NST1 + NSTC) * 8 + (NST0 + NSTC) * 4 <= 256, "too many stages");
 
     extern __shared__ __align__(128) char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const bool isA = warp < 4;
-    const int w = warp & 3;
+    const bool isA = warp < NWR;
+    const int w = isA ? warp : warp - NWR;
     const uint32_t full0 = smem_u32(smem), full1 = full0 + 8u * NST0, empty1 = full1 + 8u * NST1;
     const uint32_t fullC = empty1 + 8u * NST1;
     unsigned int* count0 = reinterpret_cast<unsigned int*>(smem + 8 * (NST0 + 2 * NST1 + NSTC));
@@ -89,7 +96,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
     char* ring1 = ringC + (size_t)NSTC * STAGEC;
     const uint32_t ring0_u32 = smem_u32(ring0), ringC_u32 = smem_u32(ringC);
     const int nx = A.nx, ny = A.ny;
-    const int tile_cells = kQuadRuns * C;
+    const int tile_cells = quad_runs(NWR) * C;
     constexpr int NBOX = 6 * NG;
     constexpr uint32_t STAGE_TX = (uint32_t)(NBOX * RB * BOXB);
 
@@ -132,12 +139,12 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
     if (threadIdx.x == 0) {
         for (int s = 0; s < NST0; ++s) { mbar_init(full0 + 8u * s, 1); count0[s] = 0u; }
         for (int s = 0; s < NSTC; ++s) { mbar_init(fullC + 8u * s, 1); countC[s] = 0u; }
-        for (int s = 0; s < NST1; ++s) { mbar_init(full1 + 8u * s, 4); mbar_init(empty1 + 8u * s, 4); }
+        for (int s = 0; s < NST1; ++s) { mbar_init(full1 + 8u * s, NWR); mbar_init(empty1 + 8u * s, NWR); }
         fence_barrier_init();
         fence_proxy_async();
     }
     // ring1 runs that no A lane writes are read (and discarded) by B's outermost lanes
-    for (int o = threadIdx.x * 16; o < NST1 * STAGE1; o += 256 * 16)
+    for (int o = threadIdx.x * 16; o < NST1 * STAGE1; o += NTHR * 16)
         *reinterpret_cast<uint4*>(ring1 + o) = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
 
@@ -152,7 +159,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
         }
     } else if constexpr (CB) {
         for (int s = 0; s < NSTC; ++s) {
-            if (warp == 4 && pc.item < A.nitems) issueC(pc, (uint32_t)s);
+            if (warp == NWR && pc.item < A.nitems) issueC(pc, (uint32_t)s);
             advance_cursor(pc);
         }
     }
@@ -163,12 +170,12 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
     const int src_arr = isA ? ARR0 : ARR1, src_row = isA ? BOXB : P1;
     // coefficient rows: A finds them in its ring0 stage (arrays 3..5); B in ring1 (arrays 3..5) or,
     // in the C builds, in its own box (same origin as ring0's boxes: run -2; the outermost lane of
-    // B warp 3 owns run 120, one past the box: it reads, and discards, the last run)
+    // the last B warp owns the run one past the box: it reads, and discards, the last run)
     const int cof_off = isA || !CB ? src_off : min((30 * w + lane + 1) * 16, BOXB - 16);
     const int cof_arr = isA || CB ? ARR0 : ARR1, cof_row = isA || CB ? BOXB : P1;
     const int dst_off = (30 * w + lane) * 16;              // A: own run in a ring1 row
     const int run0 = isA ? 30 * w - 2 + lane : 30 * w - 1 + lane;  // tile run this lane owns
-    const bool lane_ok = lane >= 1 && lane <= (isA || w < 3 ? kPairLanes : kPairLanes - 2);
+    const bool lane_ok = lane >= 1 && lane <= (isA || w < NWR - 1 ? kPairLanes : kPairLanes - 2);
     const size_t plane = (size_t)nx * ny;
 
     uint32_t gc = 0;
@@ -258,7 +265,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
                     prev = atomicAdd(&count0[s0], 1u);
                 }
                 prev = __shfl_sync(0xffffffffu, prev, 0);
-                if (prev == 3u) {
+                if (prev == (unsigned)NWR - 1u) {
                     if (lane == 0) { count0[s0] = 0u; __threadfence_block(); }
                     if (pc.item < A.nitems) issue(pc, s0);
                 }
@@ -271,7 +278,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_quad(const __grid_constant__ P
                     prev = atomicAdd(&countC[sc], 1u);
                 }
                 prev = __shfl_sync(0xffffffffu, prev, 0);
-                if (prev == 3u) {
+                if (prev == (unsigned)NWR - 1u) {
                     if (lane == 0) { countC[sc] = 0u; __threadfence_block(); }
                     if (pc.item < A.nitems) issueC(pc, sc);
                 }
