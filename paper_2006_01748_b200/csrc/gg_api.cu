@@ -616,23 +616,26 @@ int run_steps(gg_ctx* ctx, int kernel, long long n, long long every_k) {
     return GG_OK;
 }
 
+// raw: the tensor entries a, c as given, in scratch (the ping-pong copy no step has written yet
+// or will read again); b is already in place.
 template <typename T>
-int finish_tensor(gg_ctx* ctx) {
+int finish_tensor(gg_ctx* ctx, const void* raw_a, const void* raw_c) {
     // lambda_max(A) of the tensor as given, cached on the device for the step-size rule ...
     size_t seg; int nblk;
     reduce_geometry(ctx, &seg, &nblk);
     gg::gg_lambda_max_partial<T><<<nblk, gg::kDiagThreads, 0, ctx->stream>>>(
-        (const T*)ctx->coef[0], (const T*)ctx->coef[1], (const T*)ctx->coef[2], ctx->plane(), seg, ctx->d_scratch);
+        (const T*)raw_a, (const T*)ctx->coef[1], (const T*)raw_c, ctx->plane(), seg, ctx->d_scratch);
     GG_CUDA(ctx, cudaGetLastError());
     gg::gg_lambda_final<<<1, gg::kDiagThreads, 0, ctx->stream>>>(ctx->d_scratch, nblk, ctx->d_clock);
     GG_CUDA(ctx, cudaGetLastError());
-    // ... then a and c in their stored, pre-scaled form (StepCoef comment in gg_common.cuh)
+    // ... then a and c in their stored form: pre-scaled west- and south-face sums (StepCoef comment
+    // in gg_common.cuh)
     const int blocks = (int)std::min<size_t>((ctx->plane() + 255) / 256, (size_t)ctx->num_sms * 8);
-    gg::gg_scale_tensor<T><<<blocks, 256, 0, ctx->stream>>>((const T*)ctx->coef[0], (T*)ctx->coef[0], ctx->plane(),
-                                                           gg::tensor_scale_a(ctx->dx, ctx->dy));
+    gg::gg_face_tensor<T><<<blocks, 256, 0, ctx->stream>>>((const T*)raw_a, (T*)ctx->coef[0], ctx->nx, ctx->plane(), 1,
+                                                          gg::tensor_scale_a(ctx->dx, ctx->dy));
     GG_CUDA(ctx, cudaGetLastError());
-    gg::gg_scale_tensor<T><<<blocks, 256, 0, ctx->stream>>>((const T*)ctx->coef[2], (T*)ctx->coef[2], ctx->plane(),
-                                                           gg::tensor_scale_c(ctx->dx, ctx->dy));
+    gg::gg_face_tensor<T><<<blocks, 256, 0, ctx->stream>>>((const T*)raw_c, (T*)ctx->coef[2], ctx->nx, ctx->plane(), ctx->nx,
+                                                          gg::tensor_scale_c(ctx->dx, ctx->dy));
     GG_CUDA(ctx, cudaGetLastError());
     return GG_OK;
 }
@@ -752,10 +755,13 @@ static int set_tensor_impl(gg_ctx* ctx, const void* a, const void* b, const void
     if (!a || !b || !c) return fail(ctx, GG_ERR_ARG, "gg_set_tensor: NULL array");
     const void* src[3] = {a, b, c};
     ctx->have_tensor = false;
-    int rc = copy3(ctx, ctx->coef, src, ctx->plane() * ctx->esize(),
+    // a and c land in the ping-pong copy that holds no live time level (the next step overwrites
+    // it, nothing reads it before); finish_tensor turns them into the stored face sums
+    void* dst[3] = {ctx->state[ctx->cur ^ 1][0], ctx->coef[1], ctx->state[ctx->cur ^ 1][1]};
+    int rc = copy3(ctx, dst, src, ctx->plane() * ctx->esize(),
                    host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, host);
     if (rc) return rc;
-    rc = ctx->dtype == GG_F64 ? finish_tensor<double>(ctx) : finish_tensor<float>(ctx);
+    rc = ctx->dtype == GG_F64 ? finish_tensor<double>(ctx, dst[0], dst[2]) : finish_tensor<float>(ctx, dst[0], dst[2]);
     if (rc) return rc;
     ctx->have_tensor = true;
     return GG_OK;

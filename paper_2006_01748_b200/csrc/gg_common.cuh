@@ -5,7 +5,9 @@
 // and Table 2, evaluated in FLUX FORM:
 //
 //   (the code carries 2 phi and pre-scaled 2 F and folds the factors into the step coefficients and
-//    the stored tensor entries instead, see StepCoef and flux_V)
+//    the stored tensor entries instead, see StepCoef and flux_V; the tensor is stored as the FACE
+//    sums a_i-1,j + a_ij and c_i,j-1 + c_ij, which do not change in time, and U enters the V fluxes
+//    through M = 1 - U, formed once per cell)
 //   V face flux   phiE_ij = (1 - (U_ij + U_i+1,j)/2) (V_i+1,j - V_ij)          [Table 1, E entry x h^2]
 //                 phiN_ij = (1 - (U_ij + U_i,j+1)/2) (V_i,j+1 - V_ij)
 //   W cross terms G_ij = b_ij (W_i,j+1 - W_i,j-1),  H_ij = b_ij (W_i+1,j - W_i-1,j)
@@ -34,13 +36,17 @@ struct SimScalars {
 // that neither a new dt nor an adaptive dt_k changes a kernel argument (a captured graph survives
 // any dt).  The step kernels load them and round once to the arithmetic type T.
 //
-// The tensor fields are stored PRE-SCALED (gg_set_tensor): a' = a * 2dy/dx, c' = c * 2dx/dy, b as
-// given.  With G = b (W_i,j+1 - W_i,j-1), H = b (W_i+1,j - W_i-1,j) the doubled W face fluxes of the
-// header comment, divided by the cross-term weights dx/(2dy) resp. dy/(2dx), become
-//     FE' = (a'_ij + a'_i+1,j)(W_i+1,j - W_ij) + (G_ij + G_i+1,j)
-//     FN' = (c'_ij + c'_i,j+1)(W_i,j+1 - W_ij) + (H_ij + H_i,j+1)
-// and both carry the same step weight dt/(4 dx dy): one multiplication less per face, and on a
-// square mesh (2dy/dx = 2) bit-for-bit the values of the unscaled form.
+// The tensor fields are stored PRE-SCALED and PRE-SUMMED over the faces (gg_set_tensor,
+// gg_face_tensor in gg_dt.cuh): with a' = a * 2dy/dx, c' = c * 2dx/dy the workspace holds
+//     aw_ij = a'_i-1,j + a'_ij   (west face of cell ij;  aw_0j = 2 a'_0j, never used: zero flux)
+//     cs_ij = c'_i,j-1 + c'_ij   (south face of cell ij; cs_i0 = 2 c'_i0, never used)
+// and b as given.  With G = b (W_i,j+1 - W_i,j-1), H = b (W_i+1,j - W_i-1,j) the doubled W face
+// fluxes of the header comment, divided by the cross-term weights dx/(2dy) resp. dy/(2dx), become
+//     FE' = aw_i+1,j (W_i+1,j - W_ij) + (G_ij + G_i+1,j)
+//     FN' = cs_i,j+1 (W_i,j+1 - W_ij) + (H_ij + H_i,j+1)
+// and both carry the same step weight dt/(4 dx dy): two operations less per face than Table 2's
+// literal form (the face sums are time-independent), one array element per face and cell as
+// before, and bit for bit the values of summing a', c' in the kernel.
 template <typename T>
 struct StepCoef {
     T dt;     // dt
@@ -94,10 +100,13 @@ __device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf
 
 // Face fluxes carry a common factor (flux_V = 2 phi, flux_W = 2 F / cross-term weight) that
 // fold_coef puts into adx, ady and sw: fewer multiplications per face.
+// M = 1 - U: formed once per cell and time level, used by the U reaction and by the V face weights
 template <typename T>
-__device__ __forceinline__ T upd_U(const StepCoef<T>& k, T u, T w) {
-    // eq. (3) line 1: U + dt U (1-U) - d dt U W  =  U + U (dt (1-U) - d dt W)
-    return fma_(u, fma_(k.dt, sub((T)1, u), -mul(k.ddt, w)), u);
+__device__ __forceinline__ T one_minus(T u) { return sub((T)1, u); }
+template <typename T>
+__device__ __forceinline__ T upd_U(const StepCoef<T>& k, T u, T m, T w) {
+    // eq. (3) line 1: U + dt U (1-U) - d dt U W  =  U + U (dt M - d dt W),  M = 1 - U
+    return fma_(u, fma_(k.dt, m, -mul(k.ddt, w)), u);
 }
 template <typename T>
 __device__ __forceinline__ T upd_V(const StepCoef<T>& k, T v, T fe, T fw, T fn, T fs) {
@@ -110,15 +119,16 @@ __device__ __forceinline__ T upd_W(const StepCoef<T>& k, T v, T w, T fe, T fw, T
     return fma_(k.sw, sub(fe, fw), fma_(k.sw, sub(fn, fs), fma_(k.crdt, sub(v, w), w)));
 }
 template <typename T>
-__device__ __forceinline__ T flux_V(T u0, T u1, T v0, T v1) {
-    // 2 x [Table 1 face weight x h^2] x (V difference across the face, from cell 0 to cell 1)
-    return mul(sub((T)2, add(u0, u1)), sub(v1, v0));
+__device__ __forceinline__ T flux_V(T m0, T m1, T v0, T v1) {
+    // 2 x [Table 1 face weight x h^2] x (V difference across the face, from cell 0 to cell 1):
+    // 2 (1 - (U0 + U1)/2) = M0 + M1 with M = 1 - U
+    return mul(add(m0, m1), sub(v1, v0));
 }
 template <typename T>
-__device__ __forceinline__ T flux_W(T k0, T k1, T w0, T w1, T x0, T x1) {
-    // pre-scaled doubled face flux (Table 2): (k0'+k1')(w1-w0) + (x0+x1), k' = the stored a' or c',
-    // x = b x (tangential difference of W) of the two cells the face separates (see StepCoef)
-    return fma_(add(k0, k1), sub(w1, w0), add(x0, x1));
+__device__ __forceinline__ T flux_W(T kf, T w0, T w1, T x0, T x1) {
+    // pre-scaled doubled face flux (Table 2): kf (w1-w0) + (x0+x1), kf = the stored face sum aw or
+    // cs of the face, x = b x (tangential difference of W) of the two cells the face separates
+    return fma_(kf, sub(w1, w0), add(x0, x1));
 }
 // cross term b (W_+ - W_-) of one cell (G: y difference, H: x difference)
 template <typename T>

@@ -17,7 +17,8 @@
 //    (reading A6; the paper prints no formula: the RULE is "parity unpinned"), folds the
 //    coefficients and advances the clock -- all inside the captured graph, no host round trip.
 //  * gg_lambda_final: lambda_max(A) reduced once per gg_set_tensor and cached in the DevClock.
-//  * gg_scale_tensor: a, c are stored pre-scaled (StepCoef comment in gg_common.cuh).
+//  * gg_face_tensor: a, c are stored pre-scaled and summed over the faces (StepCoef comment in
+//    gg_common.cuh).
 //
 // All reductions are max/min (order-independent, exact), so dt_k is a deterministic function of
 // the stored state: the oracle's dt_k is bit-identical for fp64 storage.
@@ -146,11 +147,20 @@ gg_lambda_final(const double* __restrict__ partial, int nblk, DevClock* __restri
     if (threadIdx.x == 0) clk->lambda_max = sh[0];
 }
 
-// dst[q] = src[q] * scale, rounded once to T (dst may equal src).
+// The stored tensor (StepCoef comment in gg_common.cuh): a' = a * scale rounded once to T, then the
+// face sums  aw_ij = a'_i-1,j + a'_ij  (shift = 1: west faces)  or  cs_ij = c'_i,j-1 + c'_ij
+// (shift = nx: south faces), added in T -- exactly the sum the step kernels used to form per face
+// and step.  Cells without a neighbour on that side (i = 0 / j = 0) get 2 a'_ij: the flux through
+// a boundary face is zero whatever its coefficient.  src and dst must not overlap.
 template <typename T>
-__global__ void __launch_bounds__(256) gg_scale_tensor(const T* src, T* dst, size_t n, double scale) {
-    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x)
-        dst[q] = (T)((double)src[q] * scale);
+__global__ void __launch_bounds__(256) gg_face_tensor(const T* __restrict__ src, T* __restrict__ dst, int nx, size_t n,
+                                                      int shift, double scale) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        const bool has = shift == 1 ? (q % (size_t)nx) != 0 : q >= (size_t)nx;
+        const T k1 = (T)((double)src[q] * scale);
+        const T k0 = has ? (T)((double)src[q - (size_t)shift] * scale) : k1;
+        dst[q] = add(k0, k1);
+    }
 }
 
 }  // namespace gg

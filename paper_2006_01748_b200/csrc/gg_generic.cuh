@@ -19,9 +19,9 @@ struct GenericArgs {
     T* __restrict__ U1;        // [B][ny][nx] time k+1
     T* __restrict__ V1;
     T* __restrict__ W1;
-    const T* __restrict__ a;   // [ny][nx]
+    const T* __restrict__ a;   // [ny][nx]: aw, the west-face sums of the stored tensor (gg_common.cuh)
     const T* __restrict__ b;
-    const T* __restrict__ c;
+    const T* __restrict__ c;   // cs, the south-face sums
     const StepCoef<double>* __restrict__ coefs;  // [B], folded on the device (gg_dt.cuh)
     int nx, ny, nbatch;
 };
@@ -50,10 +50,11 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T wSW = at(W, iw, js), wSE = at(W, ie, js), wNW = at(W, iw, jn), wNE = at(W, ie, jn);
 
     // ---- V: four face fluxes (zero on boundary faces because the clamped neighbour equals the cell)
-    const T pE = flux_V(u, at(U, ie, j), v, at(V, ie, j));
-    const T pW = flux_V(at(U, iw, j), u, at(V, iw, j), v);
-    const T pN = flux_V(u, at(U, i, jn), v, at(V, i, jn));
-    const T pS = flux_V(at(U, i, js), u, at(V, i, js), v);
+    const T m = one_minus(u);
+    const T pE = flux_V(m, one_minus(at(U, ie, j)), v, at(V, ie, j));
+    const T pW = flux_V(one_minus(at(U, iw, j)), m, at(V, iw, j), v);
+    const T pN = flux_V(m, one_minus(at(U, i, jn)), v, at(V, i, jn));
+    const T pS = flux_V(one_minus(at(U, i, js)), m, at(V, i, js), v);
 
     // ---- W: cross terms at the cell and its four edge neighbours (clamped tangential differences)
     const T b0 = at(A.b, i, j);
@@ -62,11 +63,12 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     const T GW = cross(at(A.b, iw, j), wNW, wSW);
     const T HN = cross(at(A.b, i, jn), wNE, wNW);
     const T HS = cross(at(A.b, i, js), wSE, wSW);
-    const T a0 = at(A.a, i, j), c0 = at(A.c, i, j);
-    T fE = flux_W(a0, at(A.a, ie, j), w, wE, G0, GE);
-    T fW = flux_W(at(A.a, iw, j), a0, wW, w, GW, G0);
-    T fN = flux_W(c0, at(A.c, i, jn), w, wN, H0, HN);
-    T fS = flux_W(at(A.c, i, js), c0, wS, w, HS, H0);
+    // face sums: the east face of cell i is the west face of cell i+1, the north face of row j the
+    // south face of row j+1 (boundary faces: any finite value, the flux is zeroed below)
+    T fE = flux_W(at(A.a, ie, j), w, wE, G0, GE);
+    T fW = flux_W(at(A.a, i, j), wW, w, GW, G0);
+    T fN = flux_W(at(A.c, i, jn), w, wN, H0, HN);
+    T fS = flux_W(at(A.c, i, j), wS, w, HS, H0);
     // zero total normal flux through boundary faces (the cross part does not vanish by clamping)
     if (!hasE) fE = (T)0;
     if (!hasW) fW = (T)0;
@@ -74,7 +76,7 @@ __global__ void __launch_bounds__(256) gg_step_generic(GenericArgs<T> A) {
     if (!hasS) fS = (T)0;
 
     const size_t q = sim * plane + (size_t)j * nx + i;
-    A.U1[q] = upd_U(k, u, w);
+    A.U1[q] = upd_U(k, u, m, w);
     A.V1[q] = upd_V(k, v, pE, pW, pN, pS);
     A.W1[q] = upd_W(k, v, w, fE, fW, fN, fS);
 }

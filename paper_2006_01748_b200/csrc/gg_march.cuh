@@ -3,8 +3,9 @@
 // A lane owns a run of C consecutive cells of one grid row (16 bytes: C = 2 fp64 / 4 fp32 cells;
 // C = 1 for the tile-edge halo lanes of the two-step kernel) and walks up the grid one row at a
 // time.  It keeps, in registers, the extended run (west neighbour, C own cells, east neighbour)
-// of W for rows jc-1, jc, jc+1 and of U, V, a, b for rows jc, jc+1, plus c, the cross term H and
-// the south face fluxes of its own cells.  On every arriving row it evaluates the flux form of
+// of W for rows jc-1, jc, jc+1 and of M = 1 - U, V, aw, b for rows jc, jc+1, plus U, cs, the cross
+// term H and the south face fluxes of its own cells (aw, cs: the stored face sums of the tensor,
+// gg_common.cuh).  On every arriving row it evaluates the flux form of
 // Tables 1-2 (gg_common.cuh) for the centre row jc:
 //   * x faces 0..C of the run (interior ones shared by the two cells they separate; the run's
 //     outer faces are recomputed by the neighbouring lane rather than exchanged),
@@ -60,14 +61,14 @@ struct LaneMap {
 template <typename T, int C>
 struct MarchWindow {
     static constexpr int E = C + 2;
-    T wP[E], wC[E], wN[E], uC[E], uN[E], vC[E], vN[E], aC[E], aN[E], bC[E], bN[E];
-    T cC[C], cN[C], hC[C], hN[C], sV[C], sW[C];
+    T wP[E], wC[E], wN[E], mC[E], mN[E], vC[E], vN[E], aC[E], aN[E], bC[E], bN[E];
+    T uC[C], uN[C], cC[C], cN[C], hC[C], hN[C], sV[C], sW[C];
 
     __device__ __forceinline__ void clear() {
 #pragma unroll
-        for (int e = 0; e < E; ++e) wP[e] = wC[e] = uC[e] = vC[e] = aC[e] = bC[e] = (T)0;
+        for (int e = 0; e < E; ++e) wP[e] = wC[e] = mC[e] = vC[e] = aC[e] = bC[e] = (T)0;
 #pragma unroll
-        for (int c = 0; c < C; ++c) cC[c] = hC[c] = sV[c] = sW[c] = (T)0;
+        for (int c = 0; c < C; ++c) uC[c] = cC[c] = hC[c] = sV[c] = sW[c] = (T)0;
     }
 
     // Load row `rr` of the stage at `st` (arrays in the order U, V, W, a, b, c) as the arriving
@@ -76,13 +77,17 @@ struct MarchWindow {
         const char* own = st + L.oOff + rr * L.oSR;
         const char* west = st + L.wOff + rr * L.wSR;
         const char* east = st + L.eOff + rr * L.eSR;
-        T* dst[5] = {uN, vN, wN, aN, bN};
+        T* dst[5] = {mN, vN, wN, aN, bN};
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
             ld_run<T, C>(own + f * L.oSF, dst[f] + 1);
             dst[f][0] = *reinterpret_cast<const T*>(west + f * L.wSF);
             dst[f][C + 1] = *reinterpret_cast<const T*>(east + f * L.eSF);
         }
+#pragma unroll
+        for (int c = 0; c < C; ++c) uN[c] = mN[c + 1];
+#pragma unroll
+        for (int e = 0; e < E; ++e) mN[e] = one_minus(mN[e]);
         ld_run<T, C>(own + 5 * L.oSF, cN);
         // mirrored x ghosts of W (tangential difference in H at boundary cells)
         if (atW) wN[0] = wN[1];
@@ -100,15 +105,15 @@ struct MarchWindow {
         if constexpr (GHOST) {
             if (jn == 0) {
 #pragma unroll
-                for (int e = 0; e < E; ++e) { uC[e] = uN[e]; vC[e] = vN[e]; wC[e] = wN[e]; }
+                for (int e = 0; e < E; ++e) { mC[e] = mN[e]; vC[e] = vN[e]; wC[e] = wN[e]; }
 #pragma unroll
-                for (int c = 0; c < C; ++c) hC[c] = -hN[c];
+                for (int c = 0; c < C; ++c) { uC[c] = uN[c]; hC[c] = -hN[c]; }
             }
             if (jn == ny) {
 #pragma unroll
-                for (int e = 0; e < E; ++e) { uN[e] = uC[e]; vN[e] = vC[e]; wN[e] = wC[e]; }
+                for (int e = 0; e < E; ++e) { mN[e] = mC[e]; vN[e] = vC[e]; wN[e] = wC[e]; }
 #pragma unroll
-                for (int c = 0; c < C; ++c) hN[c] = -hC[c];
+                for (int c = 0; c < C; ++c) { uN[c] = uC[c]; hN[c] = -hC[c]; }
             }
         }
         T G[E];  // cross term of the x faces (rows jc-1, jc+1)
@@ -117,20 +122,20 @@ struct MarchWindow {
         T pV[C + 1], pW[C + 1];  // x faces f = 0..C (face f lies between extended cells f, f+1)
 #pragma unroll
         for (int f = 0; f <= C; ++f) {
-            pV[f] = flux_V(uC[f], uC[f + 1], vC[f], vC[f + 1]);
-            pW[f] = flux_W(aC[f], aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1]);
+            pV[f] = flux_V(mC[f], mC[f + 1], vC[f], vC[f + 1]);
+            pW[f] = flux_W(aC[f + 1], wC[f], wC[f + 1], G[f], G[f + 1]);   // aw of extended cell f+1
         }
         if (atW) { pV[0] = (T)0; pW[0] = (T)0; }
         if (atE) { pV[C] = (T)0; pW[C] = (T)0; }
         T nV[C], nW[C];  // north faces of the own cells
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-            nV[c] = flux_V(uC[c + 1], uN[c + 1], vC[c + 1], vN[c + 1]);
-            nW[c] = flux_W(cC[c], cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c]);
+            nV[c] = flux_V(mC[c + 1], mN[c + 1], vC[c + 1], vN[c + 1]);
+            nW[c] = flux_W(cN[c], wC[c + 1], wN[c + 1], hC[c], hN[c]);     // cs of the arriving row
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-            oU[c] = upd_U(k, uC[c + 1], wC[c + 1]);
+            oU[c] = upd_U(k, uC[c], mC[c + 1], wC[c + 1]);
             oV[c] = upd_V(k, vC[c + 1], pV[c + 1], pV[c], nV[c], sV[c]);
             oW[c] = upd_W(k, vC[c + 1], wC[c + 1], pW[c + 1], pW[c], nW[c], sW[c]);
         }
@@ -147,10 +152,10 @@ struct MarchWindow {
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             wP[e] = wC[e]; wC[e] = wN[e];
-            uC[e] = uN[e]; vC[e] = vN[e]; aC[e] = aN[e]; bC[e] = bN[e];
+            mC[e] = mN[e]; vC[e] = vN[e]; aC[e] = aN[e]; bC[e] = bN[e];
         }
 #pragma unroll
-        for (int c = 0; c < C; ++c) { cC[c] = cN[c]; hC[c] = hN[c]; }
+        for (int c = 0; c < C; ++c) { uC[c] = uN[c]; cC[c] = cN[c]; hC[c] = hN[c]; }
     }
 };
 

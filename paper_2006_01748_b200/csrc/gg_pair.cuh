@@ -11,8 +11,10 @@
 //    k+2 (level 2); both levels keep their rolling window (rows j-1, j of W; row j of U, V, a, b,
 //    c, H; the south face fluxes) in registers.
 //  * x-neighbours: the face between the runs of lanes l-1 and l is computed ONCE, by lane l, from
-//    lane l-1's edge values (u, v, a, w, G: warp shuffles) and handed back to lane l-1 by shuffle;
-//    the W neighbours of the tangential difference H come by shuffle too.  No neighbour loads.
+//    lane l-1's edge values (M = 1-U, V, G: warp shuffles; W: the H shuffle of one row earlier; the
+//    face's coefficient is the lane's own stored face sum) and handed back to lane l-1 by shuffle;
+//    the W neighbours of the tangential difference H come by shuffle too.  Seven shuffled values
+//    per level and row; no neighbour loads.
 //  * A warp therefore loads a 32-lane strip and, after two levels, lanes 1..30 hold valid time-k+2
 //    cells (the edge lanes lack a neighbour): strips overlap by two lanes, a warp stores 30 x 16 B
 //    = 480 contiguous bytes per row and field.  The NW strips of a CTA tile arrive in ring stages
@@ -61,39 +63,50 @@ template <typename T>
 __device__ __forceinline__ T shfl_down1(T x) { return __shfl_down_sync(0xffffffffu, x, 1); }
 
 // One time level of the in-register march: window of the centre row (and W one row below).
+// aC holds the west-face sums aw of the centre row, cN (an argument) the south-face sums cs of the
+// arriving row (gg_common.cuh); cC is carried only to hand the centre row's cs on to the next level.
 template <typename T, int C>
 struct PairLevel {
-    T wP[C], wC[C], uC[C], vC[C], aC[C], bC[C], cC[C], hC[C], sV[C], sW[C];
+    T wP[C], wC[C], uC[C], mC[C], vC[C], aC[C], bC[C], cC[C], hC[C], sV[C], sW[C];
+    T wWC;   // W of the centre row's west neighbour cell (the shuffled wNw of one row earlier)
 
     __device__ __forceinline__ void clear() {
 #pragma unroll
         for (int c = 0; c < C; ++c)
-            wP[c] = wC[c] = uC[c] = vC[c] = aC[c] = bC[c] = cC[c] = hC[c] = sV[c] = sW[c] = (T)0;
+            wP[c] = wC[c] = uC[c] = mC[c] = vC[c] = aC[c] = bC[c] = cC[c] = hC[c] = sV[c] = sW[c] = (T)0;
+        wWC = (T)0;
     }
 
     // Row `jn` arrives (own cells uN..cN); the centre row jn-1 is advanced one step into
     // oU, oV, oW and its coefficients are copied to oa, ob, oc; then the window rolls.
+    // atW / atE: the run touches the domain's west / east face (mirrored W neighbour in H);
+    // edge0: the run's face 0 lies ON a domain face (iown == 0 or iown == nx: the first run
+    // outside the east face computes, and zeroes, the east boundary face of its west neighbour).
     // All 32 lanes must call this together (warp shuffles).
     template <bool GHOST>
-    __device__ __forceinline__ void advance(int jn, int ny, bool atW, bool atE, const StepCoef<T>& k,
+    __device__ __forceinline__ void advance(int jn, int ny, bool atW, bool atE, bool edge0, const StepCoef<T>& k,
                                             T* uN, T* vN, T* wN, const T* aN, const T* bN, const T* cN,
                                             T* oU, T* oV, T* oW, T* oa, T* ob, T* oc) {
         // cross term H of the arriving row: tangential (x) difference with the lanes' neighbours
         T wNw = shfl_up1(wN[C - 1]), wNe = shfl_down1(wN[0]);
         if (atW) wNw = wN[0];
         if (atE) wNe = wN[C - 1];
-        T hN[C];
+        T hN[C], mN[C];
 #pragma unroll
-        for (int c = 0; c < C; ++c)
+        for (int c = 0; c < C; ++c) {
             hN[c] = cross(bN[c], c == C - 1 ? wNe : wN[c + 1 < C ? c + 1 : c], c == 0 ? wNw : wN[c > 0 ? c - 1 : 0]);
+            mN[c] = one_minus(uN[c]);
+        }
         if constexpr (GHOST) {
             if (jn == 0) {       // centre is ghost row -1: even mirror of row 0, H odd
 #pragma unroll
-                for (int c = 0; c < C; ++c) { uC[c] = uN[c]; vC[c] = vN[c]; wC[c] = wN[c]; hC[c] = -hN[c]; }
+                for (int c = 0; c < C; ++c) { uC[c] = uN[c]; mC[c] = mN[c]; vC[c] = vN[c]; wC[c] = wN[c]; hC[c] = -hN[c]; }
+                wWC = wNw;
             }
             if (jn == ny) {      // arriving row is ghost row ny: mirror of row ny-1
 #pragma unroll
-                for (int c = 0; c < C; ++c) { uN[c] = uC[c]; vN[c] = vC[c]; wN[c] = wC[c]; hN[c] = -hC[c]; }
+                for (int c = 0; c < C; ++c) { uN[c] = uC[c]; mN[c] = mC[c]; vN[c] = vC[c]; wN[c] = wC[c]; hN[c] = -hC[c]; }
+                wNw = wWC;
             }
         }
         T G[C];
@@ -103,38 +116,37 @@ struct PairLevel {
         // edge values, face C is lane+1's face 0
         T pV[C + 1], pW[C + 1];
         {
-            const T uW = shfl_up1(uC[C - 1]), vW = shfl_up1(vC[C - 1]), aW = shfl_up1(aC[C - 1]);
-            const T wW = shfl_up1(wC[C - 1]), GW = shfl_up1(G[C - 1]);
-            pV[0] = flux_V(uW, uC[0], vW, vC[0]);
-            pW[0] = flux_W(aW, aC[0], wW, wC[0], GW, G[0]);
+            const T mW = shfl_up1(mC[C - 1]), vW = shfl_up1(vC[C - 1]), GW = shfl_up1(G[C - 1]);
+            pV[0] = flux_V(mW, mC[0], vW, vC[0]);
+            pW[0] = flux_W(aC[0], wWC, wC[0], GW, G[0]);
         }
+        if (edge0) { pV[0] = (T)0; pW[0] = (T)0; }
 #pragma unroll
         for (int f = 1; f < C; ++f) {
-            pV[f] = flux_V(uC[f - 1], uC[f], vC[f - 1], vC[f]);
-            pW[f] = flux_W(aC[f - 1], aC[f], wC[f - 1], wC[f], G[f - 1], G[f]);
+            pV[f] = flux_V(mC[f - 1], mC[f], vC[f - 1], vC[f]);
+            pW[f] = flux_W(aC[f], wC[f - 1], wC[f], G[f - 1], G[f]);
         }
         pV[C] = shfl_down1(pV[0]);
         pW[C] = shfl_down1(pW[0]);
-        if (atW) { pV[0] = (T)0; pW[0] = (T)0; }
-        if (atE) { pV[C] = (T)0; pW[C] = (T)0; }
         T nV[C], nW[C];
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-            nV[c] = flux_V(uC[c], uN[c], vC[c], vN[c]);
-            nW[c] = flux_W(cC[c], cN[c], wC[c], wN[c], hC[c], hN[c]);
+            nV[c] = flux_V(mC[c], mN[c], vC[c], vN[c]);
+            nW[c] = flux_W(cN[c], wC[c], wN[c], hC[c], hN[c]);
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-            oU[c] = upd_U(k, uC[c], wC[c]);
+            oU[c] = upd_U(k, uC[c], mC[c], wC[c]);
             oV[c] = upd_V(k, vC[c], pV[c + 1], pV[c], nV[c], sV[c]);
             oW[c] = upd_W(k, vC[c], wC[c], pW[c + 1], pW[c], nW[c], sW[c]);
             oa[c] = aC[c]; ob[c] = bC[c]; oc[c] = cC[c];
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {  // roll
-            wP[c] = wC[c]; wC[c] = wN[c]; uC[c] = uN[c]; vC[c] = vN[c];
+            wP[c] = wC[c]; wC[c] = wN[c]; uC[c] = uN[c]; mC[c] = mN[c]; vC[c] = vN[c];
             aC[c] = aN[c]; bC[c] = bN[c]; cC[c] = cN[c]; hC[c] = hN[c]; sV[c] = nV[c]; sW[c] = nW[c];
         }
+        wWC = wNw;
     }
 };
 
@@ -247,7 +259,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_pair(const __grid_constant__ P
         const PairItem it = pair_item<RB>(A, item, tile_cells);
         const int iown = it.i0 + warp * VW + (lane - 1) * C;  // first own cell (lane 0: halo, may be < 0)
         const bool store_ok = lane_ok && iown < nx;
-        const bool atW = iown == 0, atE = iown + C == nx;
+        const bool atW = iown == 0, atE = iown + C == nx, edge0 = atW || iown == nx;
         const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
         T* gU = (T*)A.U1 + it.sim * plane + iown;
         T* gV = (T*)A.V1 + it.sim * plane + iown;
@@ -274,9 +286,9 @@ __global__ void __launch_bounds__(256, 1) gg_step_pair(const __grid_constant__ P
                 ld_run<T, C>(p + 4 * ARR, bN);
                 ld_run<T, C>(p + 5 * ARR, cN);
                 T u1[C], v1[C], w1[C], a1[C], b1[C], c1[C];   // row jn-1 at time k+1
-                L1.template advance<GHOST>(jn, ny, atW, atE, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
+                L1.template advance<GHOST>(jn, ny, atW, atE, edge0, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
                 T u2[C], v2[C], w2[C], a2[C], b2[C], c2[C];   // row jn-2 at time k+2
-                L2.template advance<GHOST>(jn - 1, ny, atW, atE, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
+                L2.template advance<GHOST>(jn - 1, ny, atW, atE, edge0, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
                 const int r = jn - 2;
                 if (store_ok && r >= it.j0 && r < it.j1) {
                     const size_t off = (size_t)r * nx;

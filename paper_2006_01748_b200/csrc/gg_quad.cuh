@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : NWR == 3 ? 2 : 3) gg_
         const PairItem it = quad_item<RB>(A, item, tile_cells);
         const int iown = it.i0 + run0 * C;               // first own cell (may lie outside the domain)
         const bool store_ok = lane_ok && iown >= 0 && iown < nx;
-        const bool atW = iown == 0, atE = iown + C == nx;
+        const bool atW = iown == 0, atE = iown + C == nx, edge0 = atW || iown == nx;
         const StepCoef<T> k = load_coef<T>(A.coefs + it.sim);
         T* gU = (T*)A.U1 + it.sim * plane + iown;
         T* gV = (T*)A.V1 + it.sim * plane + iown;
@@ -221,9 +221,9 @@ __global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : NWR == 3 ? 2 : 3) gg_
                 ld_run<T, C>(pcf + 1 * cof_arr, bN);
                 ld_run<T, C>(pcf + 2 * cof_arr, cN);
                 T u1[C], v1[C], w1[C], a1[C], b1[C], c1[C];   // row jn-1, one level up
-                L1.template advance<GHOST>(jn, ny, atW, atE, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
+                L1.template advance<GHOST>(jn, ny, atW, atE, edge0, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
                 T u2[C], v2[C], w2[C], a2[C], b2[C], c2[C];   // row jn-2, two levels up
-                L2.template advance<GHOST>(jn - 1, ny, atW, atE, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
+                L2.template advance<GHOST>(jn - 1, ny, atW, atE, edge0, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
                 if (isA) {
                     if (lane_ok) {                            // time-k+2 row jn-2 (and its coefficients)
                         char* o = dst + rr * P1;

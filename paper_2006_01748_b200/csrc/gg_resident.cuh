@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(256, 1) gg_step_resident(const ResidentArgs A)
                 // arriving row m (domain row r0-1+m): own run and the two neighbour elements
                 const char* so = src + m * pitch + own;
                 const char* co = coef + m * pitch + own;
-                T* sd[3] = {win.uN, win.vN, win.wN};
+                T* sd[3] = {win.mN, win.vN, win.wN};      // mN: raw U first, then M = 1 - U
 #pragma unroll
                 for (int f = 0; f < 3; ++f) {
                     ld_run<T, C>(so + f * ARRS, sd[f] + 1);
@@ -131,6 +131,10 @@ __global__ void __launch_bounds__(256, 1) gg_step_resident(const ResidentArgs A)
                     cd[f][C + 1] = *reinterpret_cast<const T*>(co + f * ARRS + 16);
                 }
                 ld_run<T, C>(co + 2 * ARRS, win.cN);
+#pragma unroll
+                for (int c = 0; c < C; ++c) win.uN[c] = win.mN[c + 1];
+#pragma unroll
+                for (int e = 0; e < C + 2; ++e) win.mN[e] = one_minus(win.mN[e]);
                 if (atW) win.wN[0] = win.wN[1];
                 if (atE) win.wN[C + 1] = win.wN[C];
 #pragma unroll
