@@ -188,18 +188,14 @@ int resolve_kernel(const gg_ctx* c) {
     // per-launch pipeline fill and the halo overhead, so small grids stay with shallower kernels.
     const double cells = (double)c->nx * c->ny * c->nbatch;
     // Small grids are launch-latency bound.  Grids that fit on chip run the
-    // whole call in one cooperative launch where that measured faster: fp32 up to 512^2, fp64 up
-    // to 128^2 (gg_step uses it for calls of >= kResidentMinSteps steps, STREAM2 for shorter ones).
-    if ((c->dtype == GG_F32 || cells <= 16384.0) &&
+    // whole call in one cooperative launch where that measured faster: up to 128^2 (fp64) / 256^2
+    // (fp32) cells (gg_step uses it for calls of >= kResidentMinSteps steps, STREAM2 for shorter ones).
+    if (cells <= (c->dtype == GG_F32 ? 65536.0 : 16384.0) &&
         resident_rows(c, c->bound ? (c->num_sms < 148 ? c->num_sms : 148) : 148) > 0)
         return GG_KERNEL_RESIDENT;
-    // fp64 from mid-size grids up: four steps per launch (measured ahead of the pair kernel from
-    // 512^2 to 8192^2 and on batches; a flat ~4.9 us per step below that)
-    if (c->dtype == GG_F64 && c->nx >= 236 && cells >= 65536.0) return GG_KERNEL_QUAD;
-    // fp32 (issue-bound with 4 cells per lane): two steps per launch in registers; grids up to
-    // ~1024^2 are still latency-bound per launch and run four steps per launch (768^2: 102 vs 83
-    // GLUPS, 1024^2: 141 vs 115)
-    if (c->dtype == GG_F32 && cells > 262144.0 && cells <= 1572864.0 && c->nx >= 472) return GG_KERNEL_QUAD;
+    // From mid-size grids up: four steps per launch (ahead of the pair kernel in both types from
+    // 512^2 to 8192^2 and on batches; a flat 4.5-5 us per step below ~600^2).  Needs one 58-run tile.
+    if (c->nx >= gg::quad_runs(2) * (c->dtype == GG_F64 ? 2 : 4) && cells >= 65536.0) return GG_KERNEL_QUAD;
     if (cells > 262144.0 && c->nx >= 240) return GG_KERNEL_PAIR;
     return GG_KERNEL_STREAM2;
 }

@@ -26,15 +26,16 @@
 //    so the B warps need not receive them from the A warps: their last-releasing warp fetches the
 //    B rows' own coefficient boxes by TMA (L2-hot: the A warps' TMA just read them) into a third
 //    ring.  ring1 then carries U, V, W only and the A warps shed three of their six shared-memory
-//    stores per row.  Needs one TMA box per array and row (fp64).
+//    stores per row.
 #pragma once
 #include "gg_pair.cuh"
 
 namespace gg {
 
-// NWR = warps per role (A and B): 4 (one 8-warp CTA per SM), 3 (two 6-warp CTAs per SM) or 2 (three
-// 4-warp CTAs per SM).  Narrower tiles leave registers and shared memory for more warps per SM and
-// fit grid widths that 236-cell tiles pad badly (1024 cells = 4.34 tiles of 4 warps, 5.8 of 3).
+// NWR = warps per role (A and B): 4 (one 8-warp CTA per SM) or 2 (two 4-warp CTAs per SM: the same
+// eight warps, registers and shared memory per SM).  The narrower tile fits grid widths that
+// 236-cell tiles pad badly (1024 fp64 cells = 4.34 tiles of 4 warps but 8.83 tiles of 2) at the
+// price of a little more overlap (116 output cells per 128 lanes instead of 236 per 256).
 __host__ __device__ constexpr int quad_runs(int nwr) { return 30 * nwr - 2; }        // output runs per tile row
 __host__ __device__ constexpr int quad_ring1_runs(int nwr) { return 30 * nwr + 3; }  // runs per ring1 row (run -2 ..)
 template <typename T> __host__ __device__ constexpr int quad_gw(int nwr) { return nwr < pair_gw<T>() ? nwr : pair_gw<T>(); }
@@ -66,7 +67,7 @@ __device__ __forceinline__ PairItem quad_item(const PairArgs& A, long long item,
 // [full0[NST0], full1[NST1], empty1[NST1], fullC[NSTC] mbarriers, count0[NST0], countC[NSTC];
 //  256 B][ring0: 6 arrays][ringC: a,b,c for the B warps (NSTC > 0)][ring1: U,V,W (+ a,b,c if NSTC == 0)].
 template <typename T, int RB, int NST0, int NST1, int NSTC, int NWR>
-__global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : NWR == 3 ? 2 : 3) gg_step_quad(const __grid_constant__ PairArgs A) {
+__global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : 2) gg_step_quad(const __grid_constant__ PairArgs A) {
     constexpr int C = 16 / (int)sizeof(T);
     constexpr int GW = quad_gw<T>(NWR);
     constexpr int NG = quad_ng<T>(NWR);
@@ -80,7 +81,6 @@ __global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : NWR == 3 ? 2 : 3) gg_
     constexpr int STAGEC = 3 * ARR0;
     constexpr int NTHR = 64 * NWR;
     static_assert(STAGE0 == quad_ring0_stage<T>(RB, NWR), "layout");
-    static_assert(!CB || NG == 1, "the C builds need one TMA box per array and row (fp64)");
     static_assert((NST0 + 2 * NST1 + NSTC) * 8 + (NST0 + NSTC) * 4 <= 256, "too many stages");
 
     extern __shared__ __align__(128) char smem[];
@@ -120,11 +120,12 @@ __global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : NWR == 3 ? 2 : 3) gg_
         const uint32_t bar = fullC + 8u * slot;
         const uint32_t dst = ringC_u32 + slot * STAGEC;
         const int y = pc.it.j0 - 6 + pc.q * RB;
-        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(3 * RB * BOXB));
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(3 * NG * RB * BOXB));
         __syncwarp();
-        if (lane < 3) {
-            const CUtensorMap* map = lane == 0 ? &A.ma : lane == 1 ? &A.mb : &A.mc;
-            tma_load_3d(dst + lane * ARR0, map, bar, pc.it.i0 - 2 * C, y, 0);
+        if (lane < 3 * NG) {
+            const int f = lane / NG, g = lane - NG * f;
+            const CUtensorMap* map = f == 0 ? &A.ma : f == 1 ? &A.mb : &A.mc;
+            tma_load_3d(dst + f * ARR0 + g * SLAB, map, bar, pc.it.i0 - 2 * C + g * GW * VW, y, 0);
         }
     };
     auto advance_cursor = [&](PairCursor& pc) {
@@ -169,9 +170,12 @@ __global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : NWR == 3 ? 2 : 3) gg_
                             : (30 * w + lane + 1) * 16;
     const int src_arr = isA ? ARR0 : ARR1, src_row = isA ? BOXB : P1;
     // coefficient rows: A finds them in its ring0 stage (arrays 3..5); B in ring1 (arrays 3..5) or,
-    // in the C builds, in its own box (same origin as ring0's boxes: run -2; the outermost lane of
-    // the last B warp owns the run one past the box: it reads, and discards, the last run)
-    const int cof_off = isA || !CB ? src_off : min((30 * w + lane + 1) * 16, BOXB - 16);
+    // in the C builds, in its own boxes (same origins as ring0's boxes: run -2 + 30 GW g; a run in
+    // the two-run overlap of two boxes is taken from the later one; the outermost lane of the last
+    // B warp owns the run one past the last box: it reads, and discards, that box's last run)
+    const int cof_t = 30 * w + lane + 1;                   // the B lane's run, counted from run -2
+    const int cof_g = min(cof_t / (30 * GW), NG - 1);
+    const int cof_off = isA || !CB ? src_off : cof_g * SLAB + min(cof_t - 30 * GW * cof_g, BOXB / 16 - 1) * 16;
     const int cof_arr = isA || CB ? ARR0 : ARR1, cof_row = isA || CB ? BOXB : P1;
     const int dst_off = (30 * w + lane) * 16;              // A: own run in a ring1 row
     const int run0 = isA ? 30 * w - 2 + lane : 30 * w - 1 + lane;  // tile run this lane owns

@@ -65,12 +65,12 @@ def seam_spots(wl):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config3_full_size_sampled(cfg3, dtype):
-    wl, n = cfg3, 7      # fp64: one four-step, one two-step and one single-step launch; fp32: 3 + 1
+    wl, n = cfg3, 7      # one four-step, one two-step and one single-step launch
     with binding.from_workload(wl, dtype=dtype) as sim:
-        # what AUTO resolves to, i.e. what bench.py times: fp64 four steps per launch, fp32 two
-        assert sim.kernel == ("quad" if dtype == "f64" else "pair")
+        # what AUTO resolves to, i.e. what bench.py times: four steps per launch in both types
+        assert sim.kernel == "quad"
         sim.step(n, wl.dt)
-        assert sim.launches == (n // 4 + (n % 4) // 2 + n % 2 if dtype == "f64" else n // 2 + n % 2)
+        assert sim.launches == n // 4 + (n % 4) // 2 + n % 2
         got = sim.get_state_numpy()
     for g in got:
         assert np.isfinite(g).all()
@@ -116,11 +116,11 @@ def test_config4_full_size_batch_sampled():
 def test_large_ragged_grid_sampled(dtype):
     """A grid wider than the headline one in cells per row for fp32 tiles, ragged against every
     tile width of the library (236 / 480 / 944 / 1888 cells) and against the row chunks: 10008 x
-    5001 cells, AUTO kernel, six steps (fp64: one four-step + one two-step launch)."""
+    5001 cells, AUTO kernel, six steps (one four-step + one two-step launch)."""
     wl = workloads.make(3, nx=10008, ny=5001)
     n = 6
     with binding.from_workload(wl, dtype=dtype) as sim:
-        assert sim.kernel == ("quad" if dtype == "f64" else "pair")
+        assert sim.kernel == "quad"
         sim.step(n, wl.dt)
         got = sim.get_state_numpy()
     for g in got:

@@ -318,18 +318,20 @@ def test_pair_rectangular_mesh():
 # ---------------------------------------------------------------------------------------------
 # GG_KERNEL_QUAD: four steps per launch (two register-chained pair marches linked by a ring)
 # ---------------------------------------------------------------------------------------------
-def test_quad_every_variant_and_chunking():
-    wl = workloads.random_problem(45, 488, 150, batch=2)   # fp64: 3 tiles of 236 cells, ragged
+@pytest.mark.parametrize("dtype,nx", [("f64", 488), ("f32", 976)])
+def test_quad_every_variant_and_chunking(dtype, nx):
+    # three tile columns (fp64: 236 cells each, fp32: 472), the last one ragged
+    wl = workloads.random_problem(45, nx, 150, batch=2)
     ref = {n: oracle_run(wl, n) for n in (4, 11)}
-    base = {n: gpu_run(wl, n, kernel="stream")[0] for n in (4, 11)}
+    base = {n: gpu_run(wl, n, dtype=dtype, kernel="stream")[0] for n in (4, 11)}
     for v in range(binding.gg_num_quad_variants()):
         for ipc, n in ((1, 4), (4, 11), (16, 4)):
-            got, used = gpu_run(wl, n, kernel="quad", options=[(binding.GG_OPT_QUAD_VARIANT, v),
-                                                               (binding.GG_OPT_ITEMS_PER_WARP, ipc)])
+            got, used = gpu_run(wl, n, dtype=dtype, kernel="quad",
+                                options=[(binding.GG_OPT_QUAD_VARIANT, v), (binding.GG_OPT_ITEMS_PER_WARP, ipc)])
             assert used == "quad"
-            assert_close(got, ref[n], "f64", f"quad variant {v} items/CTA {ipc}")
+            assert_close(got, ref[n], dtype, f"quad {dtype} variant {v} items/CTA {ipc}")
             for x, y in zip(got, base[n]):
-                assert np.array_equal(x, y), f"quad variant {v}: not bit-identical"
+                assert np.array_equal(x, y), f"quad {dtype} variant {v}: not bit-identical"
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
@@ -400,14 +402,15 @@ def test_resident_refuses_grids_that_do_not_fit():
 
 
 def test_user_stream_every_auto_path():
-    """The library enqueues on the stream given to gg_bind: run the resident, quad, pair and
-    generic paths on a non-default stream while the default stream is kept busy."""
+    """The library enqueues on the stream given to gg_bind: run the resident, quad (whose odd step
+    counts end with a pair and a single-step launch) and generic paths on a non-default stream
+    while the default stream is kept busy."""
     import torch
     stream = torch.cuda.Stream()
     busy = torch.empty(64 << 20, device="cuda")
     for wl, n, want, dtype in ((workloads.make(0), 40, "resident", "f64"),
                                (workloads.make(1, nx=512, ny=160, steps=1), 24, "quad", "f64"),
-                               (workloads.make(3, nx=2048, ny=800, steps=1), 10, "pair", "f32"),
+                               (workloads.make(3, nx=2048, ny=800, steps=1), 11, "quad", "f32"),
                                (workloads.make(3, nx=1200, ny=400, steps=1), 12, "quad", "f32"),
                                (workloads.random_problem(3, 41, 23), 9, "generic", "f64")):
         for _ in range(4):
