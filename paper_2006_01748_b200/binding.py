@@ -23,7 +23,8 @@ GG_OK, GG_ERR_ARG, GG_ERR_STATE, GG_ERR_CUDA, GG_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
 GG_KERNEL_AUTO, GG_KERNEL_GENERIC, GG_KERNEL_STREAM, GG_KERNEL_STREAM2, GG_KERNEL_RESIDENT, \
     GG_KERNEL_PAIR, GG_KERNEL_QUAD = range(7)
 GG_OPT_KERNEL, GG_OPT_GRAPH, GG_OPT_GRAPH_CHUNK, GG_OPT_STREAM_VARIANT, GG_OPT_ITEMS_PER_WARP, \
-    GG_OPT_STREAM_WARPS, GG_OPT_STREAM2_VARIANT, GG_OPT_PAIR_VARIANT, GG_OPT_QUAD_VARIANT = range(9)
+    GG_OPT_STREAM_WARPS, GG_OPT_STREAM2_VARIANT, GG_OPT_PAIR_VARIANT, GG_OPT_QUAD_VARIANT, \
+    GG_OPT_RESIDENT_IMPL, GG_OPT_CLUSTER_CTAS = range(11)
 
 KERNEL_NAMES = {GG_KERNEL_AUTO: "auto", GG_KERNEL_GENERIC: "generic", GG_KERNEL_STREAM: "stream",
                 GG_KERNEL_STREAM2: "stream2", GG_KERNEL_RESIDENT: "resident", GG_KERNEL_PAIR: "pair", GG_KERNEL_QUAD: "quad"}

@@ -28,6 +28,7 @@
 #include "gg_dt.cuh"
 #include "gg_tuning.h"
 #include "gg_resident.cuh"
+#include "gg_cluster.cuh"
 
 namespace {
 
@@ -90,11 +91,14 @@ struct gg_ctx {
     int opt_pair_variant = -1, opt_quad_variant = -1;
     // on-chip resident kernel (gg_resident.cuh)
     struct ResidentPlan {
-        int R = 0, slabs_per_sim = 0, grid = 0, block = 0;
+        int R = 0, slabs_per_sim = 0, grid = 0, block = 0, block_y = 1;
         size_t smem = 0;
         const void* fn = nullptr;
         bool ready = false;
+        bool cluster = false;     // gg_cluster.cuh (one cluster per simulation) instead of gg_resident.cuh
     } resident;
+    int opt_resident_impl = 0;    // tuning: 0 = cluster kernel where a simulation fits one, 1 = never
+    int opt_cluster_ctas = 0;     // tuning: CTAs per cluster (8 or 16); 0 = from the batch size
     void* d_res_halo = nullptr;
     unsigned int* d_res_flags = nullptr;
     int opt_variant2 = -1;        // -1 = tuned default for the dtype
@@ -135,6 +139,10 @@ struct Layout {
     size_t state[2][3], coef[3], sims, coefs, clock, scratch, res_halo, res_flags, total;
 };
 int resident_rows(const gg_ctx* c, int max_slabs);
+int cluster_rows(const gg_ctx* c);
+int cluster_ctas(const gg_ctx* c);
+int cluster_run_cells(const gg_ctx* c);
+bool resident_fits(const gg_ctx* c);   // either on-chip implementation can take the shape
 size_t resident_halo_bytes(const gg_ctx* c);
 // scratch for the reductions of gg_diag.cuh: [nbatch][kDiagMaxBlocks][8] partials + [nbatch][8]
 size_t scratch_doubles(const gg_ctx* c);
@@ -187,9 +195,13 @@ int resolve_kernel(const gg_ctx* c) {
     // Tuned on B200.  The deeper the temporal blocking, the larger the
     // per-launch pipeline fill and the halo overhead, so small grids stay with shallower kernels.
     const double cells = (double)c->nx * c->ny * c->nbatch;
-    // Small grids are launch-latency bound.  Grids that fit on chip run the
-    // whole call in one cooperative launch where that measured faster: up to 128^2 (fp64) / 256^2
-    // (fp32) cells (gg_step uses it for calls of >= kResidentMinSteps steps, STREAM2 for shorter ones).
+    // Small grids are latency-bound.  A simulation that fits into the shared
+    // memory of one thread-block cluster runs the whole call on chip, one cluster per simulation
+    // (gg_cluster.cuh: 64^2 fp64 0.84 us per step, 256^2 fp32 2.7), as long as the batch fills at
+    // most two waves of clusters; gg_step uses it for calls of >= kResidentMinSteps steps, STREAM2
+    // for shorter ones.  Other small shapes that fit on chip as row slabs: gg_resident.cuh.
+    if (cluster_rows(c) > 0 && c->opt_resident_impl != 1 && (long long)c->nbatch * cluster_ctas(c) <= 2 * 148)
+        return GG_KERNEL_RESIDENT;
     if (cells <= (c->dtype == GG_F32 ? 65536.0 : 16384.0) &&
         resident_rows(c, c->bound ? (c->num_sms < 148 ? c->num_sms : 148) : 148) > 0)
         return GG_KERNEL_RESIDENT;
@@ -888,7 +900,7 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
                 break;
             }
             if (value == GG_KERNEL_RESIDENT) {
-                if (resident_rows(ctx, 148) == 0)
+                if (!resident_fits(ctx))
                     return fail(ctx, GG_ERR_UNSUPPORTED, "resident kernel: %d x %d x %d does not fit on chip", ctx->nx, ctx->ny, ctx->nbatch);
                 break;
             }
@@ -912,6 +924,14 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
             if (value < 0 || value > 8)
                 return fail(ctx, GG_ERR_ARG, "GG_OPT_STREAM_WARPS: 0..8");
             break;
+        case GG_OPT_RESIDENT_IMPL:
+            if (value != 0 && value != 1) return fail(ctx, GG_ERR_ARG, "GG_OPT_RESIDENT_IMPL: 0 or 1");
+            if (value == 1 && ctx->bound && !ctx->d_res_halo)
+                return fail(ctx, GG_ERR_UNSUPPORTED, "GG_OPT_RESIDENT_IMPL = 1: the slab kernel cannot take %d x %d x %d", ctx->nx, ctx->ny, ctx->nbatch);
+            break;
+        case GG_OPT_CLUSTER_CTAS:
+            if (value != 0 && value != 2 && value != 4 && value != 8 && value != 16) return fail(ctx, GG_ERR_ARG, "GG_OPT_CLUSTER_CTAS: 0, 2, 4, 8 or 16");
+            break;
         case GG_OPT_QUAD_VARIANT:
             if (value < -1 || value >= kNumQuadVariants) return fail(ctx, GG_ERR_ARG, "GG_OPT_QUAD_VARIANT: -1 or 0..%d", kNumQuadVariants - 1);
             break;
@@ -932,6 +952,8 @@ int gg_set_option(gg_ctx* ctx, int option, long long value) {
         case GG_OPT_STREAM_WARPS: ctx->opt_warps = (int)value; ctx->plan_ready = ctx->plan2_ready = false; ctx->pair.ready = false; break;
         case GG_OPT_PAIR_VARIANT: ctx->opt_pair_variant = (int)value; ctx->pair.ready = false; break;
         case GG_OPT_QUAD_VARIANT: ctx->opt_quad_variant = (int)value; ctx->quad.ready = false; break;
+        case GG_OPT_RESIDENT_IMPL: ctx->opt_resident_impl = (int)value; ctx->resident.ready = false; break;
+        case GG_OPT_CLUSTER_CTAS: ctx->opt_cluster_ctas = (int)value; ctx->resident.ready = false; break;
     }
     return GG_OK;
 }
@@ -1018,7 +1040,10 @@ const char* gg_kernel_name(const gg_ctx* ctx) {
     try {
         switch (resolve_kernel(ctx)) {
             case GG_KERNEL_GENERIC: snprintf(buf, sizeof buf, "gg_step_generic<%s>", T); break;
-            case GG_KERNEL_RESIDENT: snprintf(buf, sizeof buf, "gg_step_resident<%s>", T); break;
+            case GG_KERNEL_RESIDENT:
+                if (cluster_rows(ctx) > 0 && ctx->opt_resident_impl != 1) snprintf(buf, sizeof buf, "gg_step_cluster<%s,%d>", T, cluster_run_cells(ctx));
+                else snprintf(buf, sizeof buf, "gg_step_resident<%s>", T);
+                break;
             case GG_KERNEL_STREAM:
                 if (!ctx->plan_ready) return "";
                 snprintf(buf, sizeof buf, "gg_step_stream<%s,%d,%d,%d>", T, ctx->plan.rb, ctx->plan.nst, ctx->plan.nw); break;

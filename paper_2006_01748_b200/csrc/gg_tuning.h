@@ -16,7 +16,10 @@ enum {
                                    PAIR 1..8; 0 = from nx                                          */
     GG_OPT_STREAM2_VARIANT = 6, /* build of the STREAM2 kernel; -1 = tuned default for the dtype   */
     GG_OPT_PAIR_VARIANT = 7,    /* build of the PAIR kernel; -1 = tuned default                    */
-    GG_OPT_QUAD_VARIANT = 8     /* build of the QUAD kernel; -1 = tuned default for the dtype      */
+    GG_OPT_QUAD_VARIANT = 8,    /* build of the QUAD kernel; -1 = tuned default for the dtype      */
+    GG_OPT_RESIDENT_IMPL = 9,   /* GG_KERNEL_RESIDENT: 0 = one cluster per simulation where it fits
+                                   (gg_cluster.cuh), 1 = always the slab kernel (gg_resident.cuh)  */
+    GG_OPT_CLUSTER_CTAS = 10    /* CTAs per cluster of gg_cluster.cuh: 2, 4, 8, 16; 0 = from the batch */
 };
 
 /* number of builds selectable with the corresponding GG_OPT_*_VARIANT */

@@ -365,28 +365,60 @@ def test_quad_configs_long_runs_bit_identical_to_single_step():
 # ---------------------------------------------------------------------------------------------
 # GG_KERNEL_RESIDENT: all n steps in one cooperative launch, state in shared memory
 # ---------------------------------------------------------------------------------------------
+# impl 0: one thread-block cluster per simulation where it fits (gg_cluster.cuh: distributed shared
+# memory, every cell of a slab in parallel); impl 1: row slabs over the whole GPU (gg_resident.cuh)
+@pytest.mark.parametrize("impl", [0, 1])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_resident_shapes_batches_and_ragged_slabs(dtype):
+def test_resident_shapes_batches_and_ragged_slabs(dtype, impl):
     for nx, ny, batch in ((4, 2, 1), (8, 3, 2), (60, 17, 3), (64, 64, 1), (124, 41, 3), (200, 297, 1),
-                          (512, 150, 1), (328, 150, 2)):
+                          (512, 150, 1), (328, 150, 2), (64, 5, 40), (128, 128, 20)):
         if dtype == "f64" and nx > 512:
             continue
+        if impl == 1 and batch > 5:
+            continue                      # more slabs than SMs: only the cluster kernel takes these
         wl = workloads.random_problem(500 + nx, nx, ny, batch=batch)
         for n in (1, 2, 9):
-            got, used = gpu_run(wl, n, dtype=dtype, kernel="resident")
+            got, used = gpu_run(wl, n, dtype=dtype, kernel="resident", options=[(binding.GG_OPT_RESIDENT_IMPL, impl)])
             assert used == "resident"
-            assert_close(got, oracle_run(wl, n), dtype, f"resident {dtype} {nx}x{ny}x{batch} n={n}")
+            assert_close(got, oracle_run(wl, n), dtype, f"resident impl {impl} {dtype} {nx}x{ny}x{batch} n={n}")
 
 
-def test_resident_long_runs_bit_identical_to_single_step():
+@pytest.mark.parametrize("impl", [0, 1])
+def test_resident_long_runs_bit_identical_to_single_step(impl):
     for wl, n in ((workloads.make(0), 200), (workloads.make(1, nx=256, ny=512, steps=400), 401),
                   (workloads.make(4, nx=264, ny=90, batch=5, steps=60), 60),
                   (workloads.random_problem(8, 328, 150, batch=2, dy_ratio=0.6), 33)):
-        a, _ = gpu_run(wl, n, kernel="resident", split=[1, 2, 0, 7, n - 10])
+        a, _ = gpu_run(wl, n, kernel="resident", split=[1, 2, 0, 7, n - 10], options=[(binding.GG_OPT_RESIDENT_IMPL, impl)])
         b, _ = gpu_run(wl, n, kernel="stream")
         for x, y in zip(a, b):
             assert np.array_equal(x, y)
-        assert_close(a, oracle_run(wl, n), "f64", f"resident {wl.name}")
+        assert_close(a, oracle_run(wl, n), "f64", f"resident impl {impl} {wl.name}")
+
+
+def test_resident_kernel_names():
+    with binding.from_workload(workloads.make(0)) as sim:
+        assert sim.kernel == "resident" and sim.kernel_name == "gg_step_cluster<double,1>"
+        sim.set_option(binding.GG_OPT_RESIDENT_IMPL, 1)
+        assert sim.kernel_name == "gg_step_resident<double>"
+
+
+def test_two_live_contexts_interleaved():
+    """Two contexts of different shapes alive at once, stepped alternately, on the kernels whose
+    dynamic shared-memory size depends on the shape (resident, cluster, pair): per-function
+    attributes must not leak from one context into the other."""
+    wa, wb = workloads.random_problem(71, 512, 96), workloads.random_problem(72, 64, 48)
+    for kernel, opts in (("resident", [(binding.GG_OPT_RESIDENT_IMPL, 1)]), ("resident", []), ("pair", [])):
+        with binding.from_workload(wa, dtype="f32") as sa, binding.from_workload(wb, dtype="f32") as sb:
+            for sim in (sa, sb):
+                sim.set_option(binding.GG_OPT_KERNEL, KERNELS[kernel])
+                for o, v in opts:
+                    sim.set_option(o, v)
+            for _ in range(3):
+                sa.step(4, wa.dt)
+                sb.step(4, wb.dt)
+            ga, gb = sa.get_state_numpy(), sb.get_state_numpy()
+        assert_close(ga, oracle_run(wa, 12), "f32", f"two contexts {kernel} (a)")
+        assert_close(gb, oracle_run(wb, 12), "f32", f"two contexts {kernel} (b)")
 
 
 def test_resident_refuses_grids_that_do_not_fit():
