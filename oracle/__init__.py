@@ -35,6 +35,14 @@ def load() -> ctypes.CDLL:
                                                     ctypes.c_int])
         lib.gg_oracle_max_threads.restype = ctypes.c_int
         lib.gg_oracle_max_threads.argtypes = []
+        # the 3-D extension (oracle/gg3_oracle.cpp)
+        lib.gg3_oracle_D1.restype = ctypes.c_int
+        lib.gg3_oracle_D1.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [_dp] * 3
+        lib.gg3_oracle_D2.restype = ctypes.c_int
+        lib.gg3_oracle_D2.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [_dp] * 8
+        lib.gg3_oracle_step.restype = ctypes.c_int
+        lib.gg3_oracle_step.argtypes = ([ctypes.c_int] * 3 + [ctypes.c_double] * 7 + [_dp] * 9 +
+                                        [ctypes.c_longlong, ctypes.c_double, ctypes.c_int])
         _lib = lib
     return _lib
 
@@ -206,3 +214,48 @@ def step_adaptive(U, V, W, a, b, c, *, r, d, alpha, c_r, n: int, safety: float, 
     if single:
         U, V, W = U[0], V[0], W[0]
     return U, V, W, t, dts
+
+
+# ---------------------------------------------------------------------------------------------
+# Three-dimensional extension.  Front for oracle/gg3_oracle.cpp:
+# the construction of eq. (3) and Tables 1-2 one dimension up (reading A13; the paper
+# prints no 3-D scheme).  Arrays are [nz][ny][nx]; the tensor is the six arrays
+# (axx, ayy, azz, axy, axz, ayz).  Pins: tests/test_oracle3d_pins.py.
+# ---------------------------------------------------------------------------------------------
+def D1_3d(U, V, dx: float, dy: float, dz: float) -> np.ndarray:
+    """Seven-point D1(V;U) (Table 1 with the two z entries added), mirrored ghosts."""
+    U, V = _c(U), _c(V)
+    nz, ny, nx = U.shape
+    out = np.empty_like(U)
+    if load().gg3_oracle_D1(nx, ny, nz, dx, dy, dz, _p(U), _p(V), _p(out)) != 0:
+        raise ValueError("gg3_oracle_D1: bad argument")
+    return out
+
+
+def D2_3d(tensor, W, dx: float, dy: float, dz: float) -> np.ndarray:
+    """Nineteen-point D2(W;A): Table 2's face and corner entries in each coordinate plane."""
+    T = [_c(t) for t in tensor]
+    W = _c(W)
+    nz, ny, nx = W.shape
+    out = np.empty_like(W)
+    if load().gg3_oracle_D2(nx, ny, nz, dx, dy, dz, *[_p(t) for t in T], _p(W), _p(out)) != 0:
+        raise ValueError("gg3_oracle_D2: bad argument")
+    return out
+
+
+def step3d(U, V, W, tensor, *, r: float, d: float, alpha: float, c_r: float, n: int, dt: float,
+           dx: float, dy: float | None = None, dz: float | None = None, threads: int = 0):
+    """n explicit Euler steps of eq. (3) in three dimensions.  Returns new (U, V, W)."""
+    dy = dx if dy is None else dy
+    dz = dx if dz is None else dz
+    U, V, W = _c(U).copy(), _c(V).copy(), _c(W).copy()
+    T = [_c(t) for t in tensor]
+    nz, ny, nx = U.shape
+    for x in (V, W, *T):
+        if x.shape != (nz, ny, nx):
+            raise ValueError("shape mismatch")
+    rc = load().gg3_oracle_step(nx, ny, nz, dx, dy, dz, r, d, alpha, c_r, *[_p(t) for t in T],
+                                _p(U), _p(V), _p(W), int(n), float(dt), int(threads))
+    if rc != 0:
+        raise ValueError("gg3_oracle_step: bad argument")
+    return U, V, W
