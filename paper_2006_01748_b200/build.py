@@ -1,7 +1,10 @@
 """Build step for libgg.so, the product's C-ABI CUDA library (include/gg.h).
 
     nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared -Xcompiler -fPIC
-         paper_2006_01748_b200/csrc/gg_api.cu -o paper_2006_01748_b200/libgg.so
+         paper_2006_01748_b200/csrc/gg_api.cu paper_2006_01748_b200/csrc/gg3_api.cu
+         -o paper_2006_01748_b200/libgg.so
+
+(gg3_api.cu: the three-dimensional extension, include/gg3.h.)
 
 nvcc cross-compiles without a GPU; the CUDA runtime is linked statically and the one driver-API
 symbol the library needs (cuTensorMapEncodeTiled) is resolved at run time through
@@ -24,7 +27,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 def sources():
     return (sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.inc")))
-            + [os.path.join(ROOT, "include", "gg.h")])
+            + [os.path.join(ROOT, "include", "gg.h"), os.path.join(ROOT, "include", "gg3.h")])
 
 
 def needs_build() -> bool:
@@ -37,7 +40,7 @@ def needs_build() -> bool:
 def command(out: str, extra=()):
     return [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++20",
             "-shared", "-Xcompiler", "-fPIC", "-cudart", "static", *extra,
-            os.path.join(CSRC, "gg_api.cu"), "-o", out]
+            os.path.join(CSRC, "gg_api.cu"), os.path.join(CSRC, "gg3_api.cu"), "-o", out]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

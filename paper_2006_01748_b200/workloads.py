@@ -266,3 +266,87 @@ def random_problem(seed: int, nx: int, ny: int, *, batch: int = 1, hetero: bool 
     return Workload(name=f"random {batch}x{nx}x{ny} seed {seed}", cfg=-1, nx=nx, ny=ny, h=h,
                     batch=batch, r=r_, d=d_, alpha=al_, c_r=cr_, a=a, b=b, c=c, U=U, V=V, W=W,
                     dt=dt, steps=8, hy=None if dy_ratio == 1.0 else hy)
+
+
+# ---------------------------------------------------------------------------------------------
+# Three-dimensional extension.  The paper prints no 3-D
+# experiment; the recipe carries config 2's into a box: a smooth heterogeneous positive-definite
+# tensor built from seeded cosine modes, a tumour BALL in healthy tissue, no acid.  Input
+# construction only (the step-size rule is the one arithmetic exception, as in 2-D).
+# ---------------------------------------------------------------------------------------------
+@dataclass
+class Workload3:
+    name: str
+    nx: int
+    ny: int
+    nz: int
+    dx: float
+    dy: float
+    dz: float
+    r: float
+    d: float
+    alpha: float
+    c_r: float
+    tensor: tuple        # (axx, ayy, azz, axy, axz, ayz), each [nz][ny][nx]
+    U: np.ndarray        # [nz][ny][nx]
+    V: np.ndarray
+    W: np.ndarray
+    dt: float
+    steps: int
+
+    @property
+    def cells(self) -> int:
+        return self.nx * self.ny * self.nz
+
+
+def dt_rule3(hmin: float, alpha: float, tensor) -> float:
+    """0.12 * hmin^2 / max(alpha, max over cells of the largest absolute row sum of A) -- Gershgorin's
+    bound on lambda_max(A); 0.12 < 1/6 keeps the seven-point diagonal part monotone in 3-D."""
+    axx, ayy, azz, axy, axz, ayz = tensor
+    rows = np.maximum(np.maximum(axx + np.abs(axy) + np.abs(axz), ayy + np.abs(axy) + np.abs(ayz)),
+                      azz + np.abs(axz) + np.abs(ayz))
+    return 0.12 * hmin * hmin / max(alpha, float(rows.max()))
+
+
+def _modes3(rng, x, y, z, L):
+    """a field in [-1, 1] from 6 seeded cosine modes with wavenumbers 1..3 over the box"""
+    f = np.zeros(np.broadcast_shapes(x.shape, y.shape, z.shape))
+    for _ in range(6):
+        kx, ky, kz = rng.integers(1, 4, 3)
+        ph = rng.uniform(0.0, 2.0 * np.pi)
+        f = f + np.cos(2.0 * np.pi * (kx * x / L[0] + ky * y / L[1] + kz * z / L[2]) + ph)
+    return f / 6.0
+
+
+def make3d(nx: int, ny: int, nz: int, *, steps: int = 10, d: float = 10.0, seed: int = 0,
+           spacing=(H, H, H), random_state: bool = False) -> Workload3:
+    """Seeded 3-D problem: diagonal entries 1e-2 (1 + f/2), off-diagonals 0.3 g sqrt(a_pp a_qq)
+    (|0.3 g| <= 0.3 on all three keeps A positive definite by Gershgorin), a tumour ball of radius
+    0.12 L centred at (0.4, 0.55, 0.5) L with V = 1, U = 0 inside, U = 1, V = 0 outside, W = 0, plus
+    uniform [0, 1e-3) noise on U then V, clipped.  random_state: uniform [0,1) fields instead (parity
+    tests on tiny or awkward shapes)."""
+    rng = np.random.default_rng([SEED, 3, nx, ny, nz, seed])
+    dx, dy, dz = spacing
+    L = (nx * dx, ny * dy, nz * dz)
+    x = ((np.arange(nx) + 0.5) * dx)[None, None, :]
+    y = ((np.arange(ny) + 0.5) * dy)[None, :, None]
+    z = ((np.arange(nz) + 0.5) * dz)[:, None, None]
+    diag = [1e-2 * (1.0 + 0.5 * _modes3(rng, x, y, z, L)) for _ in range(3)]
+    g = [_modes3(rng, x, y, z, L) for _ in range(3)]
+    axy = 0.3 * g[0] * np.sqrt(diag[0] * diag[1])
+    axz = 0.3 * g[1] * np.sqrt(diag[0] * diag[2])
+    ayz = 0.3 * g[2] * np.sqrt(diag[1] * diag[2])
+    tensor = tuple(np.ascontiguousarray(t) for t in (*diag, axy, axz, ayz))
+    shape = (nz, ny, nx)
+    if random_state:
+        U, V, W = (rng.uniform(0.0, 1.0, shape) for _ in range(3))
+    else:
+        rad = 0.12 * min(L)
+        inside = (x - 0.4 * L[0]) ** 2 + (y - 0.55 * L[1]) ** 2 + (z - 0.5 * L[2]) ** 2 <= rad * rad
+        U = np.where(inside, 0.0, 1.0) + rng.uniform(0.0, 1e-3, shape)
+        V = np.where(inside, 1.0, 0.0) + rng.uniform(0.0, 1e-3, shape)
+        U, V, W = np.clip(U, 0.0, 1.0), np.clip(V, 0.0, 1.0), np.zeros(shape)
+    alpha = 1e-3
+    return Workload3(name=f"3-D smooth heterogeneous {nx}x{ny}x{nz}", nx=nx, ny=ny, nz=nz, dx=dx, dy=dy, dz=dz,
+                     r=1.0, d=d, alpha=alpha, c_r=1.0, tensor=tensor, U=U, V=V, W=W,
+                     dt=dt_rule3(min(spacing), alpha, tensor), steps=steps)

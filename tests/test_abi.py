@@ -45,6 +45,27 @@ def test_binding_covers_exactly_the_header():
         assert callable(getattr(binding, name)), f"binding lacks a function named {name}"
 
 
+GG3_H = os.path.join(ROOT, "include", "gg3.h")
+
+
+def declared_symbols3():
+    src = re.sub(r"/\*.*?\*/", "", open(GG3_H).read(), flags=re.S)
+    return sorted(set(re.findall(r"\b(gg3_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_3d_header_exports_and_binding_agree():
+    from paper_2006_01748_b200 import binding3
+    names = declared_symbols3()
+    for need in ("gg3_create", "gg3_set_tensor", "gg3_set_state", "gg3_step", "gg3_get_state"):
+        assert need in names
+    lib = ctypes.CDLL(build.build())
+    for name in names:
+        assert hasattr(lib, name), f"libgg.so does not export {name}"
+    assert sorted(binding3.SIGNATURES) == names
+    for name in names:
+        assert callable(getattr(binding3, name)), f"binding3 lacks a function named {name}"
+
+
 def test_library_has_sm100a_code_and_tma():
     """The shipped cubin is for sm_100a and the stream kernel really uses TMA (UTMALDG in SASS)."""
     import subprocess
