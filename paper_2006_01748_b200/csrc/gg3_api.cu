@@ -85,7 +85,7 @@ int launch_step(gg3_ctx* c, int kernel, int src, double dt) {
         const dim3 block(gg3::kTileX, gg3::kTileY);
         const dim3 grid((c->nx + gg3::kTileX - 1) / gg3::kTileX, (c->ny + gg3::kTileY - 1) / gg3::kTileY,
                         gg3::tiled_zchunks(c->nx, c->ny, c->nz));
-        gg3::gg3_step_tiled<T><<<grid, block, 0, c->stream>>>(a);
+        gg3::gg3_step_tiled<T><<<grid, block, gg3::tiled_smem_bytes<T>(), c->stream>>>(a);
     } else {
         const dim3 block(32, 4, 2);
         const dim3 grid((c->nx + 31) / 32, (c->ny + 3) / 4, (c->nz + 1) / 2);
@@ -145,6 +145,8 @@ int gg3_bind(gg3_ctx* ctx, void* ws, size_t bytes, void* stream) {
     for (int f = 0; f < 6; ++f) { ctx->tens[f] = ctx->ws + off; off += array_bytes(ctx); }
     GG3_CUDA(ctx, cudaEventCreate(&ctx->ev0));
     GG3_CUDA(ctx, cudaEventCreate(&ctx->ev1));
+    GG3_CUDA(ctx, cudaFuncSetAttribute(gg3::gg3_step_tiled<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gg3::tiled_smem_bytes<double>()));
+    GG3_CUDA(ctx, cudaFuncSetAttribute(gg3::gg3_step_tiled<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gg3::tiled_smem_bytes<float>()));
     ctx->bound = true;
     return GG_OK;
 }
