@@ -22,7 +22,13 @@
 
 namespace gg3 {
 
-constexpr int kTileX = 32, kTileY = 8;
+#ifndef GG3_TILE_Y
+#define GG3_TILE_Y 2
+#endif
+#ifndef GG3_TILE_X
+#define GG3_TILE_X 64
+#endif
+constexpr int kTileX = GG3_TILE_X, kTileY = GG3_TILE_Y;
 constexpr int kPX = kTileX + 2, kPY = kTileY + 2, kPlane = kPX * kPY;   // haloed plane
 constexpr int kHalo = 2 * kPX + 2 * kTileY;                              // cells of the halo ring
 
