@@ -23,7 +23,7 @@
 namespace gg3 {
 
 #ifndef GG3_TILE_Y
-#define GG3_TILE_Y 2
+#define GG3_TILE_Y 4
 #endif
 #ifndef GG3_TILE_X
 #define GG3_TILE_X 64
@@ -31,6 +31,7 @@ namespace gg3 {
 constexpr int kTileX = GG3_TILE_X, kTileY = GG3_TILE_Y;
 constexpr int kPX = kTileX + 2, kPY = kTileY + 2, kPlane = kPX * kPY;   // haloed plane
 constexpr int kHalo = 2 * kPX + 2 * kTileY;                              // cells of the halo ring
+static_assert(kHalo <= kTileX * kTileY, "one halo cell per thread at most");
 
 __host__ __device__ inline bool tiled_shape_ok(int nx, int ny, int nz) { return nx >= 2 && ny >= 2 && nz >= 2; }
 // chunks along z: enough CTAs to fill the GPU several times over, but at least 8 planes per chunk
