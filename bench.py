@@ -414,6 +414,47 @@ def other_configs(device, wl3):
                          "tolerance": 1e-10 if dtype == "f64" else 2e-4}
         log(f"config {name}: {out[name]}")
         del wl
+    out.update(extension_3d(device))
+    return out
+
+
+def extension_3d(device):
+    """The three-dimensional extension (include/gg3.h): 256 x 256 x 256 cells of
+    the seeded 3-D recipe, AUTO kernel, fp64 and fp32; median device time of 5 repetitions of 10
+    steps; parity of a 40^3 corner window (three Neumann faces) of a separate 4-step run against
+    the 3-D oracle, recomputed from the initial data with a 4-cell margin."""
+    import torch
+    import oracle
+    from paper_2006_01748_b200 import binding3, workloads
+    peak, _ = measured_peak()
+    wl = workloads.make3d(256, 256, 256)
+    out = {}
+    for dtype, tol in (("f64", 1e-10), ("f32", 2e-4)):
+        es = 8 if dtype == "f64" else 4
+        with binding3.from_workload(wl, dtype=dtype, device=str(device)) as sim:
+            n, win = 4, 40
+            sim.step(n, wl.dt)
+            got = sim.get_state_numpy()
+            m = win + n
+            cut = lambda P: np.ascontiguousarray(P[:m, :m, :m])
+            ref = oracle.step3d(cut(wl.U), cut(wl.V), cut(wl.W), [cut(t) for t in wl.tensor], r=wl.r, d=wl.d,
+                                alpha=wl.alpha, c_r=wl.c_r, n=n, dt=wl.dt, dx=wl.dx, dy=wl.dy, dz=wl.dz)
+            err = max(float(np.max(np.abs(g[:win, :win, :win].astype(np.float64) - r[:win, :win, :win]))) for g, r in zip(got, ref))
+            K, ms = 10, []
+            sim.step(K, wl.dt)
+            for _ in range(5):
+                sim.step(K, wl.dt)
+                ms.append(sim.last_step_ms())
+            torch.cuda.synchronize(device)
+            t = float(np.median(ms))
+            glups = wl.cells * K / (t * 1e-3) / 1e9
+            out["ext3d_" + dtype] = {"workload": wl.name, "dtype": dtype, "steps": K, "kernel": "gg3_step_" + sim.kernel,
+                                     "glups": glups, "us_per_step": t * 1e3 / K,
+                                     "roofline": {"bound": "hbm", "achieved": glups * 12 * es, "peak": peak, "unit": "GB/s",
+                                                  "frac": glups * 12 * es / peak,
+                                                  "algorithmic_bytes_per_cell_step": 12 * es},
+                                     "parity_window_max_abs_err": err, "tolerance": tol}
+        log(f"config ext3d_{dtype}: {out['ext3d_' + dtype]}")
     return out
 
 

@@ -309,13 +309,18 @@ def dt_rule3(hmin: float, alpha: float, tensor) -> float:
 
 
 def _modes3(rng, x, y, z, L):
-    """a field in [-1, 1] from 6 seeded cosine modes with wavenumbers 1..3 over the box"""
+    """a field in [-1, 1] from 6 seeded cosine modes with wavenumbers 1..3 over the box:
+    cos(tx + ty + tz + ph) assembled from an xy-plane factor and a z factor (one pass per mode)"""
     f = np.zeros(np.broadcast_shapes(x.shape, y.shape, z.shape))
     for _ in range(6):
         kx, ky, kz = rng.integers(1, 4, 3)
         ph = rng.uniform(0.0, 2.0 * np.pi)
-        f = f + np.cos(2.0 * np.pi * (kx * x / L[0] + ky * y / L[1] + kz * z / L[2]) + ph)
-    return f / 6.0
+        txy = 2.0 * np.pi * (kx * x / L[0] + ky * y / L[1])          # [1][ny][nx]
+        tz = 2.0 * np.pi * kz * z / L[2] + ph                         # [nz][1][1]
+        f += np.cos(txy) * np.cos(tz)
+        f -= np.sin(txy) * np.sin(tz)
+    f /= 6.0
+    return f
 
 
 def make3d(nx: int, ny: int, nz: int, *, steps: int = 10, d: float = 10.0, seed: int = 0,
