@@ -46,7 +46,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "cell-updates/s, explicit finite-volume step, fp64 8192^2 (BASELINE config 3)"
+METRIC = "cell-updates/s, explicit finite-volume step, fp64 8192^2 (BASELINE config 3)"   # --dtype f32: labelled fp32
 UNIT = "GLUPS"
 BYTES_PER_CELL = {"f64": 72.0, "f32": 36.0}   # 3 fields read + 3 written + 3 coefficients read
 FALLBACK_HBM_GBS = 6650.0                      # /opt/skills/guides/B200_PROFILING.md
@@ -119,7 +119,8 @@ def record_traffic(raw_csv):
         pipe = "smsp__inst_executed_pipe_fp64.sum" if f64 else "smsp__inst_executed_pipe_fma.sum"
         inst = num(r, pipe)
         entry = {"traffic_bytes_per_launch": (rd + wr) * scale, "steps_per_launch": steps,
-                 "gpu_time_us_under_ncu": num(r, "gpu__time_duration.sum")}
+                 "gpu_time_under_ncu": num(r, "gpu__time_duration.sum"),
+                 "gpu_time_unit": rows[1][col["gpu__time_duration.sum"]]}
         if inst is not None:
             entry["pipe_instr_per_cell_step"] = inst * 32.0 / (8192.0 * 8192.0 * steps)
             entry["pipe_metric"] = pipe
@@ -524,7 +525,7 @@ def main():
         traffic = rec["traffic_bytes_per_launch"] if rec else None
         dram_actual = (traffic / (launch_ms * 1e-3) / 1e9) if traffic else None
         line = {
-            "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world,
+            "metric": METRIC if args.dtype == "f64" else METRIC.replace("fp64", "fp32"), "value": res["value"], "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": res["ms"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": args.dtype, "data": "synthetic",

@@ -49,6 +49,30 @@ __device__ __forceinline__ void st_run(char* p, const T* x) {
     }
 }
 
+// Predicated 16-byte stores without a branch (the row bodies of gg_quad.cuh stay one basic block).
+// No "memory" clobber on purpose: `volatile` keeps them ordered against the mbarrier operations,
+// and nothing the same thread loads later aliases what it stores here.
+template <typename T, int C>
+__device__ __forceinline__ void st_run_shared_if(bool ok, uint32_t addr, const T* x) {
+    static_assert(C * sizeof(T) == 16, "16-byte runs");
+    if constexpr (sizeof(T) == 8)
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.shared.v2.f64 [%1], {%2, %3};\n\t}"
+                     ::"r"((uint32_t)ok), "r"(addr), "d"(x[0]), "d"(x[1]));
+    else
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.shared.v4.f32 [%1], {%2, %3, %4, %5};\n\t}"
+                     ::"r"((uint32_t)ok), "r"(addr), "f"(x[0]), "f"(x[1]), "f"(x[2]), "f"(x[3]));
+}
+template <typename T, int C>
+__device__ __forceinline__ void st_run_global_if(bool ok, void* addr, const T* x) {
+    static_assert(C * sizeof(T) == 16, "16-byte runs");
+    if constexpr (sizeof(T) == 8)
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.global.v2.f64 [%1], {%2, %3};\n\t}"
+                     ::"r"((uint32_t)ok), "l"(addr), "d"(x[0]), "d"(x[1]));
+    else
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.global.v4.f32 [%1], {%2, %3, %4, %5};\n\t}"
+                     ::"r"((uint32_t)ok), "l"(addr), "f"(x[0]), "f"(x[1]), "f"(x[2]), "f"(x[3]));
+}
+
 // Where a lane finds its data inside one ring stage: byte offset of row 0 of array 0, stride per
 // array, stride per row -- for the own run and for the west / east neighbour elements (which may
 // live in the neighbour warp's strip or in a tile-edge halo slab with different strides).

@@ -228,6 +228,22 @@ __global__ void __launch_bounds__(64 * NWR, NWR == 4 ? 1 : 2) gg_step_quad(const
                 L1.template advance<GHOST>(jn, ny, atW, atE, edge0, k, uN, vN, wN, aN, bN, cN, u1, v1, w1, a1, b1, c1);
                 T u2[C], v2[C], w2[C], a2[C], b2[C], c2[C];   // row jn-2, two levels up
                 L2.template advance<GHOST>(jn - 1, ny, atW, atE, edge0, k, u1, v1, w1, a1, b1, c1, u2, v2, w2, a2, b2, c2);
+                if constexpr (CB) {
+                    // both roles' stores, predicated, no branch: the RB rows of a stage stay one
+                    // basic block, which ptxas schedules across rows (+3 % fp64, +5 % fp32 at 8192^2
+                    // over a branch per role and row)
+                    const uint32_t o = smem_u32(dst) + rr * P1;
+                    const bool sa = isA && lane_ok;
+                    st_run_shared_if<T, C>(sa, o + 0 * ARR1, u2);
+                    st_run_shared_if<T, C>(sa, o + 1 * ARR1, v2);
+                    st_run_shared_if<T, C>(sa, o + 2 * ARR1, w2);
+                    const int r = jn - 2;
+                    const bool sb = !isA && store_ok && r >= it.j0 && r < it.j1;
+                    const size_t off = (size_t)(sb ? r : 0) * nx;
+                    st_run_global_if<T, C>(sb, gU + off, u2);
+                    st_run_global_if<T, C>(sb, gV + off, v2);
+                    st_run_global_if<T, C>(sb, gW + off, w2);
+                } else
                 if (isA) {
                     if (lane_ok) {                            // time-k+2 row jn-2 (and its coefficients)
                         char* o = dst + rr * P1;
