@@ -33,6 +33,12 @@ namespace gg {
 
 constexpr int kPairLanes = 30;  // lanes of a warp that hold valid cells after two levels
 
+// fp32: arithmetic on packed pairs of cells (FADD2 / FMUL2 / FFMA2), bit-identical to the scalar code
+#ifndef GG_PACKED_F32
+#define GG_PACKED_F32 1
+#endif
+constexpr bool kPackedF32 = GG_PACKED_F32 != 0;
+
 struct alignas(64) PairArgs {
     CUtensorMap mU, mV, mW, ma, mb, mc;  // rank-3 maps {nx, ny, B}, box {GW*30*C + 2C, RB, 1}
     void* U1;
@@ -87,6 +93,10 @@ struct PairLevel {
     __device__ __forceinline__ void advance(int jn, int ny, bool atW, bool atE, bool edge0, const StepCoef<T>& k,
                                             T* uN, T* vN, T* wN, const T* aN, const T* bN, const T* cN,
                                             T* oU, T* oV, T* oW, T* oa, T* ob, T* oc) {
+        if constexpr (kPackedF32 && sizeof(T) == 4 && C == 4) {
+            advance_packed<GHOST>(jn, ny, atW, atE, edge0, k, uN, vN, wN, aN, bN, cN, oU, oV, oW, oa, ob, oc);
+            return;
+        }
         // cross term H of the arriving row: tangential (x) difference with the lanes' neighbours
         T wNw = shfl_up1(wN[C - 1]), wNe = shfl_down1(wN[0]);
         if (atW) wNw = wN[0];
@@ -143,6 +153,92 @@ struct PairLevel {
         }
 #pragma unroll
         for (int c = 0; c < C; ++c) {  // roll
+            wP[c] = wC[c]; wC[c] = wN[c]; uC[c] = uN[c]; mC[c] = mN[c]; vC[c] = vN[c];
+            aC[c] = aN[c]; bC[c] = bN[c]; cC[c] = cN[c]; hC[c] = hN[c]; sV[c] = nV[c]; sW[c] = nW[c];
+        }
+        wWC = wNw;
+    }
+
+    // fp32, four cells per lane: the same operations on PACKED pairs of cells (Blackwell's FADD2 /
+    // FMUL2 / FFMA2: two fp32 operations per instruction and issue slot).  Everything whose operands
+    // are aligned per cell -- M, G, H's product, the y faces, the three updates, the face products --
+    // runs on the pairs (cells 0,1) and (2,3); the differences and sums of x-NEIGHBOURS (shifted by
+    // one cell) stay scalar and write straight into pair halves.  Each component is rounded exactly
+    // as in the scalar code (a - b = fma(b, -1, a)), so the results are bit-identical to it.
+    template <bool GHOST>
+    __device__ __forceinline__ void advance_packed(int jn, int ny, bool atW, bool atE, bool edge0, const StepCoef<T>& k,
+                                                   T* uN, T* vN, T* wN, const T* aN, const T* bN, const T* cN,
+                                                   T* oU, T* oV, T* oW, T* oa, T* ob, T* oc) {
+        auto P = [](const T* x, int p) { return make_float2((float)x[2 * p], (float)x[2 * p + 1]); };
+        auto S = [](T* x, int p, float2 v) { x[2 * p] = (T)v.x; x[2 * p + 1] = (T)v.y; };
+        auto sub2 = [](float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); };
+        auto rep = [](T x) { return make_float2((float)x, (float)x); };
+        T wNw = shfl_up1(wN[3]), wNe = shfl_down1(wN[0]);
+        if (atW) wNw = wN[0];
+        if (atE) wNe = wN[3];
+        T hN[4], mN[4], dh[4];
+        dh[0] = sub(wN[1], wNw); dh[1] = sub(wN[2], wN[0]); dh[2] = sub(wN[3], wN[1]); dh[3] = sub(wNe, wN[2]);
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            S(hN, p, __fmul2_rn(P(bN, p), P(dh, p)));
+            S(mN, p, __ffma2_rn(P(uN, p), make_float2(-1.f, -1.f), make_float2(1.f, 1.f)));
+        }
+        if constexpr (GHOST) {
+            if (jn == 0) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { uC[c] = uN[c]; mC[c] = mN[c]; vC[c] = vN[c]; wC[c] = wN[c]; hC[c] = -hN[c]; }
+                wWC = wNw;
+            }
+            if (jn == ny) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { uN[c] = uC[c]; mN[c] = mC[c]; vN[c] = vC[c]; wN[c] = wC[c]; hN[c] = -hC[c]; }
+                wNw = wWC;
+            }
+        }
+        T G[4];
+#pragma unroll
+        for (int p = 0; p < 2; ++p) S(G, p, __fmul2_rn(P(bC, p), sub2(P(wN, p), P(wP, p))));
+        // x faces 0..3: sums and differences of x-neighbours (scalar), then the products (packed)
+        const T mW = shfl_up1(mC[3]), vW = shfl_up1(vC[3]), GW = shfl_up1(G[3]);
+        T sm[4], dv[4], dw[4], sg[4], pV[5], pW[5];
+        sm[0] = add(mW, mC[0]); dv[0] = sub(vC[0], vW); dw[0] = sub(wC[0], wWC); sg[0] = add(GW, G[0]);
+#pragma unroll
+        for (int f = 1; f < 4; ++f) {
+            sm[f] = add(mC[f - 1], mC[f]); dv[f] = sub(vC[f], vC[f - 1]);
+            dw[f] = sub(wC[f], wC[f - 1]); sg[f] = add(G[f - 1], G[f]);
+        }
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            S(pV, p, __fmul2_rn(P(sm, p), P(dv, p)));
+            S(pW, p, __ffma2_rn(P(aC, p), P(dw, p), P(sg, p)));
+        }
+        if (edge0) { pV[0] = (T)0; pW[0] = (T)0; }
+        pV[4] = shfl_down1(pV[0]);
+        pW[4] = shfl_down1(pW[0]);
+        T dpv[4], dpw[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { dpv[c] = sub(pV[c + 1], pV[c]); dpw[c] = sub(pW[c + 1], pW[c]); }
+        const float2 kdt = rep(k.dt), knd = rep(-k.ddt), krd = rep(k.rdt), kax = rep(k.adx), kay = rep(k.ady),
+                     kcr = rep(k.crdt), ksw = rep(k.sw);
+        T nV[4], nW[4];
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            const float2 u = P(uC, p), m = P(mC, p), v = P(vC, p), w = P(wC, p);
+            // north faces
+            const float2 nv = __fmul2_rn(__fadd2_rn(m, P(mN, p)), sub2(P(vN, p), v));
+            const float2 nw = __ffma2_rn(P(cN, p), sub2(P(wN, p), w), __fadd2_rn(P(hC, p), P(hN, p)));
+            S(nV, p, nv);
+            S(nW, p, nw);
+            // eq. (3): same nesting as upd_U / upd_V / upd_W
+            S(oU, p, __ffma2_rn(u, __ffma2_rn(kdt, m, __fmul2_rn(knd, w)), u));
+            const float2 rv = __ffma2_rn(__fmul2_rn(krd, v), __ffma2_rn(v, make_float2(-1.f, -1.f), make_float2(1.f, 1.f)), v);
+            S(oV, p, __ffma2_rn(kax, P(dpv, p), __ffma2_rn(kay, sub2(nv, P(sV, p)), rv)));
+            const float2 rw = __ffma2_rn(kcr, sub2(v, w), w);
+            S(oW, p, __ffma2_rn(ksw, P(dpw, p), __ffma2_rn(ksw, sub2(nw, P(sW, p)), rw)));
+        }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            oa[c] = aC[c]; ob[c] = bC[c]; oc[c] = cC[c];
             wP[c] = wC[c]; wC[c] = wN[c]; uC[c] = uN[c]; mC[c] = mN[c]; vC[c] = vN[c];
             aC[c] = aN[c]; bC[c] = bN[c]; cC[c] = cN[c]; hC[c] = hN[c]; sV[c] = nV[c]; sW[c] = nW[c];
         }
