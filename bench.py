@@ -113,11 +113,21 @@ def record_traffic(raw_csv):
         name = m.group(1)
         f64 = "<double" in name
         steps = 4 if "quad" in name else 2 if ("pair" in name or "stream2" in name) else 1
-        rd, wr = num(r, "dram__bytes_read.sum"), num(r, "dram__bytes_write.sum")
-        unit_rd = rows[1][col["dram__bytes_read.sum"]]
-        scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(unit_rd, 1.0)
+        scale_of = lambda m: {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(rows[1][col[m]], 1.0)
+        rd = num(r, "dram__bytes_read.sum") * scale_of("dram__bytes_read.sum")
+        wr = num(r, "dram__bytes_write.sum") * scale_of("dram__bytes_write.sum")
+        scale = 1.0
         pipe = "smsp__inst_executed_pipe_fp64.sum" if f64 else "smsp__inst_executed_pipe_fma.sum"
         inst = num(r, pipe)
+        if inst is None:
+            # `--set full` has the pipe's utilisation but not its instruction count: warp
+            # instructions = utilisation x peak rate (fp64: 1 per 2 cycles and SM sub-partition,
+            # fma: 1 per cycle) x active cycles x 592 sub-partitions
+            pct = num(r, ("sm__inst_executed_pipe_fp64" if f64 else "sm__inst_executed_pipe_fma") + ".avg.pct_of_peak_sustained_active")
+            cyc = num(r, "smsp__cycles_active.avg")
+            if pct is not None and cyc is not None:
+                inst = pct / 100.0 * (0.5 if f64 else 1.0) * cyc * 592.0
+                pipe += " (derived from the pipe's pct_of_peak_sustained_active)"
         entry = {"traffic_bytes_per_launch": (rd + wr) * scale, "steps_per_launch": steps,
                  "gpu_time_under_ncu": num(r, "gpu__time_duration.sum"),
                  "gpu_time_unit": rows[1][col["gpu__time_duration.sum"]]}
