@@ -68,10 +68,13 @@ enum {
     GG_KERNEL_STREAM = 2,   /* TMA-staged shared-memory row ring, register-rolling y march;     */
                             /* needs nx*sizeof(elem) % 16 == 0                                  */
     GG_KERNEL_STREAM2 = 3,  /* as STREAM with two time steps fused per launch (temporal block)  */
-    GG_KERNEL_RESIDENT = 4, /* all n steps of a call in ONE cooperative launch, state resident in */
-                            /* shared memory, row slabs exchange edge rows point-to-point; grids */
-                            /* of at most 148 slabs with rows <= 4096 B (gg_resident.cuh).  AUTO  */
-                            /* uses it for calls of >= 8 steps and STREAM2 for shorter ones       */
+    GG_KERNEL_RESIDENT = 4, /* all n steps of a call in ONE launch, state resident in shared     */
+                            /* memory: one thread-block cluster per simulation with halo rows    */
+                            /* through distributed shared memory where a simulation fits one     */
+                            /* (gg_cluster.cuh), else row slabs over the whole GPU exchanging    */
+                            /* edge rows point-to-point (cooperative launch; at most 148 slabs   */
+                            /* with rows <= 4096 B; gg_resident.cuh).  AUTO uses it for calls of */
+                            /* >= 8 steps and STREAM2 for shorter ones                           */
     GG_KERNEL_PAIR = 5,     /* two time steps per launch chained in REGISTERS, x-neighbours by  */
                             /* warp shuffle (gg_pair.cuh); needs nx*sizeof(elem) % 16 == 0      */
     GG_KERNEL_QUAD = 6      /* FOUR time steps per launch: two register-chained pair marches    */
