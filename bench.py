@@ -397,7 +397,7 @@ def window_parity(wl, final, K, s=0, size=48):
     return worst
 
 
-def other_configs(device, wl3):
+def other_configs(device, wl3, only=None):
     """The other BASELINE.json configs with AUTO kernel selection, inputs resident in HBM: median
     device time of 5 repetitions of K steps (K scaled to the config), and window parity of the end
     state of ONE K-step run against the oracle.  Builder-side numbers become driver-side ones."""
@@ -408,6 +408,8 @@ def other_configs(device, wl3):
             ("cfg4_batch64", lambda: workloads.make(4), "f64", 40), ("cfg1", lambda: workloads.make(1), "f64", 400),
             ("cfg0", lambda: workloads.make(0), "f64", 200)]
     for name, mk, dtype, K in plan:
+        if only and name != only:
+            continue
         wl = mk()
         with binding.from_workload(wl, dtype=dtype, device=str(device)) as sim:
             sim.step(K, wl.dt)
@@ -425,11 +427,12 @@ def other_configs(device, wl3):
                          "tolerance": 1e-10 if dtype == "f64" else 2e-4}
         log(f"config {name}: {out[name]}")
         del wl
-    out.update(extension_3d(device))
+    if not only or only.startswith("ext3d"):
+        out.update(extension_3d(device, only))
     return out
 
 
-def extension_3d(device):
+def extension_3d(device, only=None):
     """The three-dimensional extension (include/gg3.h): 256 x 256 x 256 cells of
     the seeded 3-D recipe, AUTO kernel, fp64 and fp32; median device time of 5 repetitions of 10
     steps; parity of a 40^3 corner window (three Neumann faces) of a separate 4-step run against
@@ -441,6 +444,8 @@ def extension_3d(device):
     wl = workloads.make3d(256, 256, 256)
     out = {}
     for dtype, tol in (("f64", 1e-10), ("f32", 2e-4)):
+        if only and only != "ext3d_" + dtype:
+            continue
         es = 8 if dtype == "f64" else 4
         with binding3.from_workload(wl, dtype=dtype, device=str(device)) as sim:
             n, win = 4, 40
@@ -484,6 +489,10 @@ def main():
     ap.add_argument("--n", type=int, default=8192, help="grid edge (8192 = the headline config)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-configs", action="store_true", help="skip the `configs` object (other BASELINE configs)")
+    ap.add_argument("--only-config", dest="only_config", default=None, metavar="NAME",
+                    help="run ONE entry of the `configs` object (cfg3_f32, cfg2_d10, cfg4_batch64, cfg1, cfg0, "
+                         "ext3d_f64, ext3d_f32), print it as a JSON line and exit: the short command the ncu "
+                         "captures of those kernels are taken with")
     ap.add_argument("--extras", action="store_true",
                     help="also time gg_diagnostics / gg_step_adaptive (adds a `reductions` object)")
     ap.add_argument("--record-traffic", default=None, metavar="RAW.csv",
@@ -515,6 +524,10 @@ def main():
         import torch.distributed as td
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         td.init_process_group("nccl", device_id=device)
+    if args.only_config:
+        wl3 = workloads.make(3) if args.only_config == "cfg3_f32" else None
+        print(json.dumps({"configs": other_configs(device, wl3, args.only_config)}), flush=True)
+        return 0
     wl = workloads.make(3, nx=args.n, ny=args.n)
     log(f"[rank {rank}] workload {wl.name}, dt={wl.dt:.6e}")
     res = run_ours(args, wl, rank, world, device)

@@ -16,16 +16,22 @@
 //    directly from shared memory: the run's C + 1 x faces once each, the 2 C y faces.  No march,
 //    no register window: the depth of a step is one run, whatever the slab height.  The CTA is
 //    two-dimensional (runs of a row x rows), so no index arithmetic is left in the step loop.
-//  * A thread on the slab's first / last row also stores its result into the neighbour CTA's halo
-//    row through distributed shared memory (mapa + st.shared::cluster).  One cluster barrier per
-//    step (barrier.cluster.arrive.release / wait.acquire) separates the time levels: no global
-//    memory, no flags, no L2 round trip between the first load and the last store of a call.
+//  * A thread on the slab's first / last row also sends its result into the neighbour CTA's halo
+//    row through distributed shared memory: `st.async ... mbarrier::complete_tx::bytes` on the
+//    NEIGHBOUR's mbarrier of that state copy.  A step ends with a CTA barrier (own rows) and a wait
+//    on the CTA's own mbarrier (both neighbours' edge rows have landed): point to point, no
+//    cluster-wide barrier in the step loop (one per step cost 0.2 us more), no global memory, no
+//    flags, no L2 round trip between the first load and the last store of a call.  A neighbour can
+//    only be one step ahead (it needs this CTA's edge row to go on), and what it then writes is
+//    the halo of the OTHER state copy, which this CTA's edge threads finished reading before
+//    they sent: the two copies and two mbarriers (one per copy, armed one round ahead) suffice.
 //  * Arithmetic: the per-cell formulas of gg_generic.cuh (clamped neighbours, boundary W fluxes
 //    zeroed) through the same functions with the same operands => bit-identical to every other
 //    kernel of the library.
 #pragma once
 #include "gg_common.cuh"
 #include "gg_march.cuh"
+#include "gg_stream.cuh"   // mbarrier wrappers
 
 namespace gg {
 
@@ -42,7 +48,7 @@ struct ClusterArgs {
 
 __host__ __device__ constexpr int cluster_pitch(int nx, int esize) { return nx * esize + 32; }
 __host__ __device__ constexpr size_t cluster_smem_bytes(int nx, int esize, int R) {
-    return (size_t)9 * (R + 2) * cluster_pitch(nx, esize);   // 2 x (U,V,W) + (aw,b,cs)
+    return (size_t)9 * (R + 2) * cluster_pitch(nx, esize) + 64;   // 2 x (U,V,W) + (aw,b,cs) + two mbarriers
 }
 
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -56,18 +62,21 @@ __device__ __forceinline__ uint32_t cluster_map(uint32_t addr, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
     return r;
 }
-// one run (4, 8 or 16 bytes) into another CTA's shared memory
+// one run (4, 8 or 16 bytes) into another CTA's shared memory, completing its byte count on that
+// CTA's mbarrier when it lands
 template <int BYTES>
-__device__ __forceinline__ void st_cluster_run(uint32_t addr, const void* x) {
+__device__ __forceinline__ void st_async_run(uint32_t addr, const void* x, uint32_t mbar) {
     if constexpr (BYTES == 16) {
         const uint4 v = *reinterpret_cast<const uint4*>(x);
-        asm volatile("st.shared::cluster.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
-                     : "memory");
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+                     ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "r"(mbar) : "memory");
     } else if constexpr (BYTES == 8) {
         const uint2 v = *reinterpret_cast<const uint2*>(x);
-        asm volatile("st.shared::cluster.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(v.x), "r"(v.y) : "memory");
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b32 [%0], {%1, %2}, [%3];"
+                     ::"r"(addr), "r"(v.x), "r"(v.y), "r"(mbar) : "memory");
     } else {
-        asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(addr), "r"(*reinterpret_cast<const uint32_t*>(x)) : "memory");
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                     ::"r"(addr), "r"(*reinterpret_cast<const uint32_t*>(x)), "r"(mbar) : "memory");
     }
 }
 __device__ __forceinline__ void cluster_barrier() {
@@ -100,6 +109,20 @@ __global__ void __launch_bounds__(512, 1) gg_step_cluster(const ClusterArgs A) {
     const bool atW = l == 0, atE = l == lanes - 1;
     const int o = 16 + RUNB * l;                              // byte offset of the run in a shared-memory row
 
+    // hbar[b]: "the halo rows of state copy b are complete" -- expects, per round, the bytes of the
+    // edge rows the neighbour CTAs send (3 fields x one row each), armed by thread 0 one round ahead
+    const uint32_t hbar = smem_u + 3 * SET;
+    const bool has_below = rows > 0 && rank > 0, has_above = rows > 0 && r1 < ny;
+    const uint32_t halo_tx = (uint32_t)(((has_below ? 1 : 0) + (has_above ? 1 : 0)) * 3 * nx * ES);
+    if (tid == 0) {
+        mbar_init(hbar, 1);
+        mbar_init(hbar + 8, 1);
+        fence_barrier_init();
+        if (halo_tx != 0u) {                    // (a CTA without neighbours never touches them)
+            mbar_expect_tx(hbar + 8, halo_tx);  // round of step 0 (fills copy 1)
+            mbar_expect_tx(hbar, halo_tx);      // round of step 1 (fills copy 0)
+        }
+    }
     // ---- start-up: zero everything, then load the slab and the halo rows inside the domain
     for (int q = tid * 16; q < 3 * SET; q += nthr * 16)
         *reinterpret_cast<uint4*>(smem + q) = make_uint4(0u, 0u, 0u, 0u);
@@ -203,19 +226,30 @@ __global__ void __launch_bounds__(512, 1) gg_step_cluster(const ClusterArgs A) {
             // edge rows also go into the neighbour CTAs' halo rows (distributed shared memory)
             if (r == 0 && rank > 0) {                       // bottom row -> top halo (row R+1) of the CTA below
                 const uint32_t ra = cluster_map(smem_u + dset + (R + 1) * pitch + o, (uint32_t)(rank - 1));
-                st_cluster_run<RUNB>(ra + 0 * ARRS, oU);
-                st_cluster_run<RUNB>(ra + 1 * ARRS, oV);
-                st_cluster_run<RUNB>(ra + 2 * ARRS, oW);
+                const uint32_t rb = cluster_map(hbar + 8u * (uint32_t)((step + 1) & 1), (uint32_t)(rank - 1));
+                st_async_run<RUNB>(ra + 0 * ARRS, oU, rb);
+                st_async_run<RUNB>(ra + 1 * ARRS, oV, rb);
+                st_async_run<RUNB>(ra + 2 * ARRS, oW, rb);
             }
             if (r == rows - 1 && r1 < ny) {                 // top row -> bottom halo (row 0) of the CTA above
                 const uint32_t ra = cluster_map(smem_u + dset + o, (uint32_t)(rank + 1));
-                st_cluster_run<RUNB>(ra + 0 * ARRS, oU);
-                st_cluster_run<RUNB>(ra + 1 * ARRS, oV);
-                st_cluster_run<RUNB>(ra + 2 * ARRS, oW);
+                const uint32_t rb = cluster_map(hbar + 8u * (uint32_t)((step + 1) & 1), (uint32_t)(rank + 1));
+                st_async_run<RUNB>(ra + 0 * ARRS, oU, rb);
+                st_async_run<RUNB>(ra + 1 * ARRS, oV, rb);
+                st_async_run<RUNB>(ra + 2 * ARRS, oW, rb);
             }
         }
-        cluster_barrier();
+        // own rows of the new level: a CTA barrier; the neighbours' edge rows: this copy's mbarrier
+        // (its phase flips every second step).  Thread 0 then arms it for its next round, two
+        // steps on -- before this CTA sends anything a neighbour could answer with that round.
+        __syncthreads();
+        if (halo_tx != 0u) {
+            const uint32_t hb = hbar + 8u * (uint32_t)((step + 1) & 1);
+            mbar_wait(hb, (uint32_t)((step >> 1) & 1));
+            if (tid == 0) mbar_expect_tx(hb, halo_tx);
+        }
     }
+    cluster_barrier();   // nobody leaves while a neighbour may still be sending to it
 
     // ---- the call's last time level goes back to HBM
     {
