@@ -29,6 +29,7 @@
 #include "gg_tuning.h"
 #include "gg_resident.cuh"
 #include "gg_cluster.cuh"
+#include "gg_inst.h"
 
 namespace {
 
@@ -233,49 +234,9 @@ constexpr Variant kVariants[] = {{2, 4}, {4, 2}};
 constexpr int kNumVariants = (int)(sizeof(kVariants) / sizeof(kVariants[0]));
 constexpr int kDefaultVariant = 1;
 
-template <typename T, int RB, int NST, typename F>
-int with_nw(int nw, F&& f) {
-    switch (nw) {
-        case 1: return f.template operator()<T, RB, NST, 1>();
-        case 2: return f.template operator()<T, RB, NST, 2>();
-        case 4: return f.template operator()<T, RB, NST, 4>();
-        case 8: return f.template operator()<T, RB, NST, 8>();
-    }
-    return -1;
-}
-// Calls f.template operator()<T, RB, NST, NW>() for tuning index v and nw warps per CTA.
-template <typename T, typename F>
-int with_variant(int v, int nw, F&& f) {
-    switch (v) {
-        case 0: return with_nw<T, 2, 4>(nw, f);
-        case 1: return with_nw<T, 4, 2>(nw, f);
-    }
-    return -1;
-}
-
-// Two-step kernel builds: (rows per box, ring0 stages, ring1 stages); NW in {1, 2, 4} warps per
-// step (so 2*NW + 2 warps per CTA).  Index 0 is the fp64 default, 1 the fp32 default.
 struct Variant2 { int rb, nst0, nst1; };
 constexpr Variant2 kVariants2[] = {{4, 2, 2}, {3, 2, 2}};
 constexpr int kNumVariants2 = (int)(sizeof(kVariants2) / sizeof(kVariants2[0]));
-
-template <typename T, int RB, int N0, int N1, typename F>
-int with_nw2(int nw, F&& f) {
-    switch (nw) {
-        case 1: return f.template operator()<T, RB, N0, N1, 1>();
-        case 2: return f.template operator()<T, RB, N0, N1, 2>();
-        case 4: return f.template operator()<T, RB, N0, N1, 4>();
-    }
-    return -1;
-}
-template <typename T, typename F>
-int with_variant2(int v, int nw, F&& f) {
-    switch (v) {
-        case 0: return with_nw2<T, 4, 2, 2>(nw, f);
-        case 1: return with_nw2<T, 3, 2, 2>(nw, f);
-    }
-    return -1;
-}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
@@ -341,16 +302,6 @@ void plan_chunks(const gg_ctx* c, long long per, long long resident, int halo_ro
     *nchunks = (c->ny + *chunk_rows - 1) / *chunk_rows;
 }
 
-struct KernelPtr {
-    const void** out;
-    template <typename T, int RB, int NST, int NW>
-    int operator()() const { *out = (const void*)gg::gg_step_stream<T, RB, NST, NW>; return 0; }
-};
-struct Kernel2Ptr {
-    const void** out;
-    template <typename T, int RB, int N0, int N1, int NW>
-    int operator()() const { *out = (const void*)gg::gg_step_stream2<T, RB, N0, N1, NW>; return 0; }
-};
 // Builds the plan of the single-step (two_step = false) or two-step stream kernel.
 int build_plan(gg_ctx* c, bool two_step) {
     bool& ready = two_step ? c->plan2_ready : c->plan_ready;
@@ -392,17 +343,15 @@ int build_plan(gg_ctx* c, bool two_step) {
         if (rc) return rc;
     }
     const void* fn = nullptr;
-    int rc;
+    int rc = 0;
     if (two_step) {
         P.block = (2 * nw + 2) * 32;  // nw step-1 + nw step-2 warps, halo warp, TMA producer warp
         P.smem = (size_t)gg::stream2_smem_bytes(P.rb, P.nst, P.nst1, nw);
-        rc = c->dtype == GG_F64 ? with_variant2<double>(v2, nw, Kernel2Ptr{&fn})
-                                : with_variant2<float>(v2, nw, Kernel2Ptr{&fn});
+        fn = gg::stream2_kernel(c->dtype == GG_F64, v2, nw);
     } else {
         P.block = (nw + 1) * 32;  // nw consumer warps + the TMA producer warp
         P.smem = (size_t)gg::stream_smem_bytes(P.rb, P.nst, nw);
-        rc = c->dtype == GG_F64 ? with_variant<double>(c->opt_variant, nw, KernelPtr{&fn})
-                                : with_variant<float>(c->opt_variant, nw, KernelPtr{&fn});
+        fn = gg::stream_kernel(c->dtype == GG_F64, c->opt_variant, nw);
     }
     if (rc || !fn) return fail(c, GG_ERR_UNSUPPORTED, "no stream kernel build for this variant with %d warps", nw);
     P.fn = fn;
