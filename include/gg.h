@@ -74,7 +74,7 @@ enum {
                             /* (gg_cluster.cuh), else row slabs over the whole GPU exchanging    */
                             /* edge rows point-to-point (cooperative launch; at most 148 slabs   */
                             /* with rows <= 4096 B; gg_resident.cuh).  AUTO uses it for calls of */
-                            /* >= 8 steps and STREAM2 for shorter ones                           */
+                            /* >= 4 (cluster) resp. >= 8 (slabs) steps, STREAM2 for shorter ones */
     GG_KERNEL_PAIR = 5,     /* two time steps per launch chained in REGISTERS, x-neighbours by  */
                             /* warp shuffle (gg_pair.cuh); needs nx*sizeof(elem) % 16 == 0      */
     GG_KERNEL_QUAD = 6      /* FOUR time steps per launch: two register-chained pair marches    */

@@ -765,7 +765,8 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
         if (n == 0) return GG_OK;
         int kernel = resolve_kernel(ctx);
         const bool autosel = ctx->opt_kernel == GG_KERNEL_AUTO;
-        if (kernel == GG_KERNEL_RESIDENT && autosel && n < kResidentMinSteps)
+        if (kernel == GG_KERNEL_RESIDENT && autosel &&
+            n < (cluster_rows(ctx) > 0 && ctx->opt_resident_impl != 1 ? kClusterMinSteps : kResidentMinSteps))
             kernel = GG_KERNEL_STREAM2;   // a cooperative launch does not pay for a handful of steps
         if (kernel == GG_KERNEL_RESIDENT) {
             const int rc = build_plan_resident(ctx);

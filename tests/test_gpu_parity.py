@@ -19,13 +19,14 @@ KERNELS = {"generic": binding.GG_KERNEL_GENERIC, "stream": binding.GG_KERNEL_STR
            "quad": binding.GG_KERNEL_QUAD, "resident": binding.GG_KERNEL_RESIDENT}
 
 
-def expected_launches(kernel, calls, explicit=True):
+def expected_launches(kernel, calls, explicit=True, min_steps=8):
     """Kernel launches for a list of gg_step(n) calls: stream2 / pair advance two steps per launch,
     quad four (then two, then one), resident all n steps of a call (under AUTO only for calls of
-    at least 8 steps; shorter ones run stream2)."""
+    at least `min_steps` steps -- 4 for the cluster kernel, 8 for the slab kernel; shorter ones run
+    stream2)."""
     two = lambda n: n // 2 + n % 2
     if kernel == "resident":
-        return sum((1 if n > 0 else 0) if (explicit or n >= 8) else two(n) for n in calls)
+        return sum((1 if n > 0 else 0) if (explicit or n >= min_steps) else two(n) for n in calls)
     if kernel == "quad":
         return sum(n // 4 + (n % 4) // 2 + n % 2 for n in calls)
     if kernel in ("stream2", "pair"):
@@ -49,10 +50,11 @@ def gpu_run(wl, steps, dtype="f64", kernel=None, options=(), split=None, check_l
         for n in (split or [steps]):
             sim.step(n, wl.dt)
         used = sim.kernel
+        min_steps = 4 if "cluster" in sim.kernel_name else 8
         launches = sim.launches
         out = sim.get_state_numpy()
     if check_launches:   # (graph chunks shorter than a call split it like separate calls)
-        assert launches == expected_launches(used, split or [steps], explicit=kernel is not None)
+        assert launches == expected_launches(used, split or [steps], explicit=kernel is not None, min_steps=min_steps)
     return out, used
 
 
