@@ -51,3 +51,34 @@ def test_fuzz_all_kernels_bounded():
                 (dtype, nx, ny, batch, n, ratio, name, "differs from generic")
         ncase += 1
     print(f"fuzz: {ncase} cases")
+
+
+def test_onchip_kernels_many_calls_bit_identical():
+    """The on-chip kernels (one cluster per simulation with st.async halo rows where it fits, row
+    slabs otherwise) over calls of 1, 7, 64 and 301 steps on random small shapes and batches, bit
+    for bit against the single-step kernel: a lost or early halo hand-off changes bits."""
+    rng = np.random.default_rng(5)
+    ncase = 0
+    for it in range(16):
+        nx = int(rng.choice([8, 16, 32, 64, 96, 128, 160]))
+        ny = int(rng.integers(2, 150))
+        b = int(rng.choice([1, 1, 2, 5, 9, 20]))
+        dtype = str(rng.choice(["f64", "f32"]))
+        wl = workloads.random_problem(1000 + it, nx, ny, batch=b)
+        outs = []
+        for kern in ("resident", "stream"):
+            with B.from_workload(wl, dtype=dtype) as sim:
+                try:
+                    sim.set_option(B.GG_OPT_KERNEL, KERNELS[kern])
+                except B.GGError:
+                    outs = None
+                    break
+                for n in (1, 7, 64, 301):
+                    sim.step(n, wl.dt)
+                outs.append(sim.get_state_numpy())
+        if outs is None:
+            continue
+        ncase += 1
+        for x, y in zip(*outs):
+            assert np.array_equal(x, y), f"on-chip kernel differs from stream: {nx}x{ny}x{b} {dtype}"
+    assert ncase >= 8
