@@ -520,3 +520,18 @@ def test_mass_conservation_on_gpu():
     got, _ = gpu_run(wl, 200)
     assert abs(got[2].sum() - wl.W.sum()) <= 1e-12 * wl.W.sum()
     assert abs(got[1].sum() - wl.V.sum()) <= 1e-12 * wl.V.sum()
+
+
+def test_fp32_packed_arithmetic_keeps_denormals():
+    """The fp32 four-step kernel computes on packed pairs of cells (FADD2 / FMUL2 / FFMA2); the
+    single-step kernel is scalar.  Far from the tumour the acid field decays into the denormal
+    range: the packed instructions must round those exactly as the scalar ones (no flush to zero)."""
+    wl = workloads.random_problem(77, 944, 64)
+    wl.W *= 1e-39                       # denormal in fp32
+    wl.V *= 1e-38
+    wl.U[:] = 1.0 - 1e-7 * wl.U
+    a, _ = gpu_run(wl, 12, dtype="f32", kernel="quad")
+    b, _ = gpu_run(wl, 12, dtype="f32", kernel="stream")
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    assert np.any((np.abs(a[2]) > 0) & (np.abs(a[2]) < 1.1754944e-38))   # denormals really occur
