@@ -177,6 +177,39 @@ enum {
 };
 int gg_diagnostics(gg_ctx* ctx, double eps, double* out);
 
+/* The same nine diagnostics for a caller that has NO context, NO workspace and NO way to allocate
+ * one.  gg_diagnostics needs a context bound to caller-allocated device memory; a monitoring hook
+ * that some other program's time loop hands bare device pointers to (an in-situ probe, a plug-in
+ * of an application whose memory pool already owns the whole GPU) has no allocator to ask, and a
+ * cudaMalloc of its own may fail or, where it works, synchronises the device and stalls the loop
+ * it is watching.  This call allocates nothing, on the host side of the API or the device side:
+ * no cudaMalloc / cudaFree / allocating library routine.  Its per-block partial results live in a
+ * fixed 1.3 MiB array that is part of libgg.so's device image, present on every GPU that loads
+ * the library for the life of the process (csrc/gg_noalloc.cu).
+ *   U, V, W   DEVICE arrays [nbatch][ny][nx] of `dtype` (GG_F64 / GG_F32) on the current device,
+ *             element-aligned (16-byte alignment enables the wide loads); read only;
+ *   nbatch    1 .. GG_NOALLOC_MAX_BATCH -- the built-in array is sized for that many simulations;
+ *             more is refused with GG_ERR_ARG (split the batch, or use gg_diagnostics).  nx, ny >= 1,
+ *             any size;
+ *   eps       gap threshold, finite and >= 0;
+ *   out       DEVICE array [nbatch][GG_DIAG_COUNT] of doubles, slot order GG_DIAG_*, written by the
+ *             kernel; the caller owns it and reads it after ordering with `cuda_stream`;
+ *   cuda_stream  a cudaStream_t cast to void* (NULL = legacy default stream).  The call enqueues
+ *             one memset of a few counters and ONE kernel on it and returns without synchronising.
+ * Values: the sums are accumulated in double in a fixed order (deterministic from call to call);
+ * they agree with gg_diagnostics to summation order (~1e-15 relative), counts and extrema exactly.
+ * Sharing: every call on a GPU uses the same built-in array.  Calls on one stream are safe (the
+ * stream orders them; nothing is carried from one call to the next -- the counters are re-zeroed
+ * by every call).  Calls that may OVERLAP on the GPU (different streams or threads) race on it and
+ * give wrong results: order them yourself.
+ * First call on each GPU: looks up the array's device address and makes the runtime load the
+ * library's kernels there; make it once with that GPU current, outside any stream capture.
+ * Errors: GG_OK or a code; the message is per host thread, from gg_noalloc_last_error(). */
+enum { GG_NOALLOC_MAX_BATCH = 64 };
+int gg_diagnostics_noalloc(const void* U, const void* V, const void* W, int nbatch, int nx, int ny,
+                           int dtype, double eps, double* out, void* cuda_stream);
+const char* gg_noalloc_last_error(void);
+
 /* Front position along a grid line (the paper reads the tumour and acid fronts and the gap between
  * them off the fields): for every simulation the first and the last cell index
  * along row `index` (axis 0: the line runs along x) or column `index` (axis 1: along y) where

@@ -55,6 +55,9 @@ SIGNATURES = {
     "gg_set_state_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_get_state_host": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "gg_diagnostics": (ctypes.c_int, [_vp, ctypes.c_double, _dp]),
+    "gg_diagnostics_noalloc": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                              ctypes.c_int, ctypes.c_double, _vp, _vp]),
+    "gg_noalloc_last_error": (ctypes.c_char_p, []),
     "gg_max_stable_dt": (ctypes.c_int, [_vp, ctypes.c_double, _dp, _dp]),
     "gg_front": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                 ctypes.POINTER(ctypes.c_int)]),
@@ -191,6 +194,24 @@ def gg_diagnostics(ctx, eps: float, nbatch: int) -> np.ndarray:
     out = np.empty((nbatch, GG_DIAG_COUNT), dtype=np.float64)
     _check(ctx, load().gg_diagnostics(ctx, float(eps), out.ctypes.data_as(_dp)))
     return out
+
+
+GG_NOALLOC_MAX_BATCH = 64
+
+
+def gg_noalloc_last_error() -> str:
+    return (load().gg_noalloc_last_error() or b"").decode()
+
+
+def gg_diagnostics_noalloc(U_ptr, V_ptr, W_ptr, nbatch: int, nx: int, ny: int, dtype: int, eps: float,
+                           out_ptr, stream_ptr: int = 0):
+    """The context-free, allocation-free diagnostics call for callers that cannot allocate device
+    memory (gg.h): U, V, W and `out` ([nbatch][GG_DIAG_COUNT] doubles) are DEVICE pointers the
+    caller owns; the result is in `out` once `stream_ptr` has reached this point.  Enqueues only."""
+    rc = load().gg_diagnostics_noalloc(U_ptr, V_ptr, W_ptr, int(nbatch), int(nx), int(ny), int(dtype),
+                                       float(eps), out_ptr, stream_ptr)
+    if rc != GG_OK:
+        raise GGError(rc, gg_noalloc_last_error())
 
 
 def gg_front(ctx, field: int, axis: int, index: int, level: float, nbatch: int) -> np.ndarray:

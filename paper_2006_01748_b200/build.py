@@ -2,10 +2,11 @@
 
     nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -Xcompiler -fPIC -Xfatbin -compress-all
          -c --threads 6
-         csrc/gg_api.cu csrc/gg3_api.cu csrc/gg_inst_{quad,pair,stream,stream2}.cu
+         csrc/gg_api.cu csrc/gg3_api.cu csrc/gg_noalloc.cu csrc/gg_inst_{quad,pair,stream,stream2}.cu
     nvcc -shared -cudart static *.o -o paper_2006_01748_b200/libgg.so
 
-(gg3_api.cu: the three-dimensional extension, include/gg3.h; gg_inst_*.cu: the builds of the step
+(gg3_api.cu: the three-dimensional extension, include/gg3.h; gg_noalloc.cu: the allocation-free
+diagnostics call with its built-in device scratch; gg_inst_*.cu: the builds of the step
 kernels, one translation unit per family so that they compile in parallel.)
 
 nvcc cross-compiles without a GPU; the CUDA runtime is linked statically and the one driver-API
@@ -26,8 +27,8 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgg.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # translation units: the two ABIs and one per family of step-kernel builds (compiled in parallel)
-TUS = [os.path.join(CSRC, f) for f in ("gg_api.cu", "gg3_api.cu", "gg_inst_quad.cu", "gg_inst_pair.cu",
-                                       "gg_inst_stream.cu", "gg_inst_stream2.cu")]
+TUS = [os.path.join(CSRC, f) for f in ("gg_api.cu", "gg3_api.cu", "gg_noalloc.cu", "gg_inst_quad.cu",
+                                       "gg_inst_pair.cu", "gg_inst_stream.cu", "gg_inst_stream2.cu")]
 
 
 def sources():
