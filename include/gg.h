@@ -29,6 +29,8 @@
  * and hands it over with gg_bind; it must stay alive until gg_destroy.  All array arguments
  * marked DEVICE are device pointers on the current CUDA device; HOST are host pointers.  The
  * caller keeps ownership of every array it passes; the library copies in/out of its workspace.
+ * (One call, gg_diagnostics_noalloc, takes no workspace: its small scratch is a fixed array inside
+ * the library's own device image -- see there.)
  *
  * Streams.  Every call enqueues on the stream given to gg_bind (a cudaStream_t cast to void*,
  * NULL = the legacy default stream) and returns without synchronising, except gg_destroy,
@@ -126,7 +128,9 @@ int gg_set_state(gg_ctx* ctx, const void* U, const void* V, const void* W);
 /* n >= 0 explicit Euler steps of eq. (3) with constant step dt > 0.  All
  * three fields advance together from time-k data only.  n == 0 is a no-op.  dt is handed to the
  * device in front of the step loop and is not part of any cached graph: a new dt on every call
- * (the paper's host loop) re-captures nothing. */
+ * (the paper's host loop) re-captures nothing.  If the call fails with GG_ERR_CUDA after
+ * its first launch, state and clock no longer describe one time level: the context drops its state
+ * (later step/get calls return GG_ERR_STATE) until gg_set_state loads one again. */
 int gg_step(gg_ctx* ctx, long long n, double dt);
 
 /* n >= 0 steps with the NON-UNIFORM step size dt_k of PAPER.md:62 ("computed after each iteration
@@ -139,12 +143,22 @@ int gg_step(gg_ctx* ctx, long long n, double dt);
  * batch, held for the every_k steps that follow (the last group may be shorter).  safety > 0.
  * The reductions are exact (max / min), so dt_k is a deterministic function of the stored state.
  * GG_KERNEL_RESIDENT cannot change dt inside its single launch: GG_ERR_UNSUPPORTED if it was
- * selected explicitly (AUTO runs STREAM2 on such grids instead).  Enqueues and returns. */
+ * selected explicitly (AUTO runs STREAM2 on such grids instead).  Enqueues and returns.
+ * The rule bounds the two DIFFUSION operators only; it knows nothing of the reaction terms
+ * (d W dt, r dt, c dt of eq. (1)), whose stiffness is the caller's to cover with `safety`.
+ * When the rule has no positive finite bound (a zero tensor with alpha == 0 or U >= 1 everywhere, a
+ * non-finite tensor entry, no finite U) the device does not fold inf or NaN into the step: the
+ * steps of that group run with dt = 0 (state and simulated time stay put, the step count still
+ * advances), and the next gg_get_clock returns GG_ERR_ARG with the details; from then on gg_step
+ * and gg_step_adaptive refuse the context until gg_set_state.  (The call itself cannot report it:
+ * it returns before the device has evaluated anything.) */
 int gg_step_adaptive(gg_ctx* ctx, long long n, double safety, long long every_k);
 
 /* The device-side clock: simulated time (the sum of the step sizes of all steps since the last
  * gg_set_state), the step size of the most recent step, and the number of steps since
- * gg_set_state.  Any of the three pointers may be NULL.  Synchronises the bound stream. */
+ * gg_set_state.  Any of the three pointers may be NULL.  Synchronises the bound stream.  Returns
+ * GG_ERR_ARG (after filling the outputs) if a gg_step_adaptive since the last gg_set_state found
+ * no usable step size -- see there. */
 int gg_get_clock(gg_ctx* ctx, double* time, double* dt, long long* steps);
 
 /* Copy the current state (after every step issued so far) into DEVICE arrays [nbatch][ny][nx]. */
@@ -243,7 +257,7 @@ int gg_set_option(gg_ctx* ctx, int option, long long value);
  *                 event.  *ms < 0 if no step has run. */
 int gg_kernel_used(const gg_ctx* ctx);
 /* Name of the kernel instantiation behind gg_kernel_used, as a profiler prints it, e.g.
- * "gg_step_quad<double,4,2,2,2>" (context-owned; "" before the first gg_step built its plan). */
+ * "gg_step_quad<double,4,2,2,2,4>" (context-owned; "" before the first gg_step built its plan). */
 const char* gg_kernel_name(const gg_ctx* ctx);
 long long gg_launches(const gg_ctx* ctx);
 long long gg_graph_captures(const gg_ctx* ctx);

@@ -61,6 +61,7 @@ struct gg_ctx {
     size_t ws_bytes = 0;
     cudaStream_t stream = nullptr;
     bool bound = false, have_tensor = false, have_state = false;
+    bool rule_failed = false;   // gg_get_clock saw DevClock::bad_rule != 0; cleared by gg_set_state
     void* state[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
     void* coef[3] = {nullptr, nullptr, nullptr};
     gg::SimScalars* d_sims = nullptr;
@@ -737,6 +738,7 @@ static int set_state_impl(gg_ctx* ctx, const void* U, const void* V, const void*
     gg::gg_clock_reset<<<1, 1, 0, ctx->stream>>>(ctx->d_clock);
     GG_CUDA(ctx, cudaGetLastError());
     ctx->have_state = true;
+    ctx->rule_failed = false;
     return GG_OK;
 }
 static int get_state_impl(gg_ctx* ctx, void* U, void* V, void* W, bool host) {
@@ -760,6 +762,7 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
     return guarded(ctx, "gg_step", [&]() -> int {
         if (!ctx->bound || !ctx->have_tensor || !ctx->have_state)
             return fail(ctx, GG_ERR_STATE, "gg_step: needs gg_bind, gg_set_tensor and gg_set_state first");
+        if (ctx->rule_failed) return fail(ctx, GG_ERR_ARG, "gg_step: an earlier gg_step_adaptive found no usable step size (see gg_get_clock); call gg_set_state");
         if (n < 0) return fail(ctx, GG_ERR_ARG, "gg_step: n = %lld < 0", n);
         if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, GG_ERR_ARG, "gg_step: dt must be finite and > 0");
         if (n == 0) return GG_OK;
@@ -784,14 +787,17 @@ int gg_step(gg_ctx* ctx, long long n, double dt) {
             ctx->folded_dt == dt ? 0 : 1);
         GG_CUDA(ctx, cudaGetLastError());
         ctx->folded_dt = dt;
+        // From here on the device clock already counts all n steps: if a launch, a capture or a
+        // replay below fails, clock and state no longer belong together -- the state is dropped
+        // (gg_set_state starts over and resets the clock) rather than left looking valid.
         if (kernel == GG_KERNEL_RESIDENT) {
             const int rc = launch_resident(ctx, ctx->cur, n);
-            if (rc) return rc;
+            if (rc) { ctx->have_state = false; return rc; }
             ctx->cur ^= 1;
             ctx->launches += 1;
         } else {
             const int rc = run_steps(ctx, kernel, n, 0);
-            if (rc) return rc;
+            if (rc) { ctx->have_state = false; return rc; }
         }
         GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
         ctx->timed = true;
@@ -804,6 +810,7 @@ int gg_step_adaptive(gg_ctx* ctx, long long n, double safety, long long every_k)
     return guarded(ctx, "gg_step_adaptive", [&]() -> int {
         if (!ctx->bound || !ctx->have_tensor || !ctx->have_state)
             return fail(ctx, GG_ERR_STATE, "gg_step_adaptive: needs gg_bind, gg_set_tensor and gg_set_state first");
+        if (ctx->rule_failed) return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: an earlier call found no usable step size (see gg_get_clock); call gg_set_state");
         if (n < 0) return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: n = %lld < 0", n);
         if (!(safety > 0.0) || !std::isfinite(safety)) return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: safety must be finite and > 0");
         if (every_k < 1 || every_k > 4096) return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: every_k must be in 1..4096");
@@ -822,7 +829,7 @@ int gg_step_adaptive(gg_ctx* ctx, long long n, double safety, long long every_k)
         GG_CUDA(ctx, cudaGetLastError());
         ctx->folded_dt = std::numeric_limits<double>::quiet_NaN();   // the device decides from here on
         rc = run_steps(ctx, kernel, n, every_k);
-        if (rc) return rc;
+        if (rc) { ctx->have_state = false; return rc; }   // as in gg_step: no half-advanced state is kept
         GG_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
         ctx->timed = true;
         return GG_OK;
@@ -838,6 +845,12 @@ int gg_get_clock(gg_ctx* ctx, double* time, double* dt, long long* steps) {
     if (time) *time = h.time;
     if (dt) *dt = h.dt;
     if (steps) *steps = h.steps;
+    if (h.bad_rule != 0) {
+        ctx->rule_failed = true;
+        return fail(ctx, GG_ERR_ARG, "gg_step_adaptive: the step-size rule had no positive finite bound in %lld evaluation(s) "
+                    "(max(lambda_max, alpha (1 - min U)) = %g); those steps ran with dt = 0.  gg_set_state clears this",
+                    h.bad_rule, h.rate);
+    }
     return GG_OK;
 }
 

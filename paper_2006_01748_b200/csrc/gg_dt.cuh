@@ -34,7 +34,10 @@ struct DevClock {
     double rate;          // adaptive: the max(...) of the last dt_k rule evaluation
     double safety;        // adaptive: the safety factor of the rule (set in front of the replay)
     long long steps;      // steps taken since gg_set_state
-    long long pad_[2];
+    long long bad_rule;   // adaptive: evaluations of the dt_k rule that gave no usable step size since
+                          // gg_set_state (sticky; the steps of such a group run with dt = 0, i.e. leave
+                          // the state as it is, and gg_get_clock reports the failure)
+    long long pad_[1];
 };
 
 // dt by value (gg_step): fold every simulation's coefficients, advance the clock by n steps.
@@ -56,6 +59,7 @@ __global__ void gg_clock_reset(DevClock* __restrict__ clk) {
     clk->time = 0.0;
     clk->steps = 0;
     clk->rate = 0.0;
+    clk->bad_rule = 0;
 }
 __global__ void gg_clock_safety(DevClock* __restrict__ clk, double safety) { clk->safety = safety; }
 
@@ -120,7 +124,15 @@ gg_fold_adaptive(DevClock* __restrict__ clk, const SimScalars* __restrict__ sims
     if (threadIdx.x == 0) {
         const double rate = fmax(clk->lambda_max, sh[0]);
         const double hmin = dx < dy ? dx : dy;
-        const double dt = __ddiv_rn(__dmul_rn(__dmul_rn(clk->safety, hmin), hmin), rate);
+        double dt = __ddiv_rn(__dmul_rn(__dmul_rn(clk->safety, hmin), hmin), rate);
+        // No usable bound (A == 0 with U >= 1 everywhere, alpha == 0 with a zero tensor, a non-finite
+        // tensor entry, a state without one finite U): do not fold inf / NaN / a negative dt into
+        // the coefficients.  The group's steps run with dt = 0 (the state stays what it is, the
+        // clock's time does not move) and the failure is counted for gg_get_clock to report.
+        if (!(rate > 0.0) || !isfinite(rate) || !(dt > 0.0) || !isfinite(dt)) {
+            dt = 0.0;
+            clk->bad_rule += 1;
+        }
         clk->rate = rate;
         clk->dt = dt;
         clk->time += dt * (double)k;

@@ -50,27 +50,35 @@ __device__ __forceinline__ void st_run(char* p, const T* x) {
 }
 
 // Predicated 16-byte stores without a branch (the row bodies of gg_quad.cuh stay one basic block).
-// No "memory" clobber on purpose: `volatile` keeps them ordered against the mbarrier operations,
-// and nothing the same thread loads later aliases what it stores here.
+// They carry a "memory" clobber: the compiler is TOLD they write memory, so it can neither hoist a
+// later load of the ring above them nor sink them below the mbarrier arrive that publishes the
+// row -- the A-warp -> B-warp hand-off of gg_quad.cuh no longer rests on `volatile` ordering alone.
+// (-DGG_ST_NO_CLOBBER builds the round-2 form without it, for A/B timing; both forms are
+// bit-identical in the fuzz.)
+#ifdef GG_ST_NO_CLOBBER
+#define GG_ST_CLOBBER
+#else
+#define GG_ST_CLOBBER : "memory"
+#endif
 template <typename T, int C>
 __device__ __forceinline__ void st_run_shared_if(bool ok, uint32_t addr, const T* x) {
     static_assert(C * sizeof(T) == 16, "16-byte runs");
     if constexpr (sizeof(T) == 8)
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.shared.v2.f64 [%1], {%2, %3};\n\t}"
-                     ::"r"((uint32_t)ok), "r"(addr), "d"(x[0]), "d"(x[1]));
+                     ::"r"((uint32_t)ok), "r"(addr), "d"(x[0]), "d"(x[1]) GG_ST_CLOBBER);
     else
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.shared.v4.f32 [%1], {%2, %3, %4, %5};\n\t}"
-                     ::"r"((uint32_t)ok), "r"(addr), "f"(x[0]), "f"(x[1]), "f"(x[2]), "f"(x[3]));
+                     ::"r"((uint32_t)ok), "r"(addr), "f"(x[0]), "f"(x[1]), "f"(x[2]), "f"(x[3]) GG_ST_CLOBBER);
 }
 template <typename T, int C>
 __device__ __forceinline__ void st_run_global_if(bool ok, void* addr, const T* x) {
     static_assert(C * sizeof(T) == 16, "16-byte runs");
     if constexpr (sizeof(T) == 8)
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.global.v2.f64 [%1], {%2, %3};\n\t}"
-                     ::"r"((uint32_t)ok), "l"(addr), "d"(x[0]), "d"(x[1]));
+                     ::"r"((uint32_t)ok), "l"(addr), "d"(x[0]), "d"(x[1]) GG_ST_CLOBBER);
     else
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.global.v4.f32 [%1], {%2, %3, %4, %5};\n\t}"
-                     ::"r"((uint32_t)ok), "l"(addr), "f"(x[0]), "f"(x[1]), "f"(x[2]), "f"(x[3]));
+                     ::"r"((uint32_t)ok), "l"(addr), "f"(x[0]), "f"(x[1]), "f"(x[2]), "f"(x[3]) GG_ST_CLOBBER);
 }
 
 // Where a lane finds its data inside one ring stage: byte offset of row 0 of array 0, stride per

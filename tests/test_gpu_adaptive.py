@@ -152,6 +152,35 @@ def test_clock_counts_fixed_steps_and_resets_on_set_state():
             sim.step_adaptive(4, 0.2, 0)
 
 
+def test_adaptive_rule_without_a_bound_freezes_the_state_and_is_reported():
+    """A zero tensor with alpha = 0 leaves the rule dt = safety h^2 / max(lambda_max, alpha (1 - min U))
+    without a positive denominator.  The device must not fold inf or NaN into the step: those steps
+    run with dt = 0 (state and simulated time untouched), gg_get_clock reports GG_ERR_ARG, further
+    step calls are refused, and gg_set_state puts the context back to work."""
+    w = adaptive_problem(66, 96, 40, 2, [0.0, 0.0])
+    zero = np.zeros_like(w.a)
+    with binding.from_workload(w) as sim:
+        sim.set_tensor(zero, zero, zero)
+        before = sim.get_state_numpy()
+        sim.step_adaptive(6, 0.2, 2)                    # enqueues: the failure shows on the device
+        after = sim.get_state_numpy()
+        for b, a in zip(before, after):
+            assert np.array_equal(b, a)
+        with pytest.raises(binding.GGError) as e:
+            sim.clock()
+        assert e.value.code == binding.GG_ERR_ARG and "no positive finite bound in 3 evaluation" in str(e.value)
+        for call in (lambda: sim.step(1, 1e-3), lambda: sim.step_adaptive(1, 0.2, 1)):
+            with pytest.raises(binding.GGError) as e:
+                call()
+            assert e.value.code == binding.GG_ERR_ARG
+        sim.set_state(w.U, w.V, w.W)                    # clears the flag on both sides
+        assert sim.clock()[0] == 0.0 and sim.clock()[2] == 0
+        sim.step(2, 1e-3)
+        t, dt, steps = sim.clock()
+        assert steps == 2 and dt == 1e-3 and t == pytest.approx(2e-3, rel=1e-15)
+        assert not np.array_equal(sim.get_state_numpy()[0], before[0])
+
+
 def test_two_live_contexts_of_different_shapes_share_kernels():
     """The opt-in shared-memory limit is a per-FUNCTION attribute: a second context with a smaller
     shape must not lower it under a first context's feet (resident and pair instantiations)."""
