@@ -342,7 +342,7 @@ def run_ours(args, wl, rank, world, device):
     final = tuple(out[k].numpy() for k in ("U", "V", "W"))
     kernel, kernel_name = sim.kernel, sim.kernel_name
     reductions = None
-    if args.extras:
+    if not args.no_extras:
         # the device-side reductions next to the step: one pass over
         # U, V, W; wall clock around the synchronising C-ABI call (includes the launch and the
         # result copy), median of 7.  And the adaptive step loop: dt_k re-evaluated on the device
@@ -356,14 +356,46 @@ def run_ours(args, wl, rank, world, device):
                 ts.append(time.perf_counter() - t0)
             return float(np.median(ts))
         t_diag = timed(lambda: sim.diagnostics(1e-2))
+        t_dtmax = timed(lambda: sim.max_stable_dt(0.2))
+        # gg_diagnostics_noalloc on caller-held copies of the fields: device time of the ONE kernel
+        # (plus its counter memset) by CUDA events on torch's current stream, which is the stream
+        # the call is given; median of 7
+        Ud, Vd, Wd = sim.get_state()
+        dout = torch.empty((wl.batch, binding.GG_DIAG_COUNT), dtype=torch.float64, device=device)
+        cur = torch.cuda.current_stream(device)
+        na = []
+        for _ in range(8):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(cur)
+            binding.gg_diagnostics_noalloc(Ud.data_ptr(), Vd.data_ptr(), Wd.data_ptr(), wl.batch, wl.nx, wl.ny,
+                                           sim.dtype, 1e-2, dout.data_ptr(), int(cur.cuda_stream))
+            e1.record(cur)
+            e1.synchronize()
+            na.append(e0.elapsed_time(e1))
+        t_na = float(np.median(na[1:])) * 1e-3
+        na_same = bool(np.allclose(dout.cpu().numpy(), sim.diagnostics(1e-2), rtol=1e-12, atol=1e-12))
+        del Ud, Vd, Wd
         sim.step_adaptive(K, 0.2, 4)
         ad = []
         for _ in range(5):
             sim.step_adaptive(K, 0.2, 4)
             ad.append(sim.last_step_ms())
-        reductions = {"gg_diagnostics_ms": t_diag * 1e3, "gg_diagnostics_gbs": 3 * cells * es / t_diag / 1e9,
-                      "bound": "hbm", "bytes": "3 arrays read once, 24 B (fp64) / 12 B (fp32) per cell",
-                      "gg_step_adaptive_every_4_glups": cells * K / (float(np.median(ad)) * 1e-3) / 1e9}
+        peak_gbs, _ = measured_peak()
+        gbs = lambda t: 3 * cells * es / t / 1e9
+        reductions = {"bound": "hbm", "bytes": "3 arrays read once, 24 B (fp64) / 12 B (fp32) per cell",
+                      "timing": "gg_diagnostics / gg_max_stable_dt: wall clock around the synchronising C-ABI call "
+                                "(launches + result copy included), median of 7; gg_diagnostics_noalloc: CUDA events "
+                                "around the enqueue-only call, median of 7",
+                      "gg_diagnostics_ms": t_diag * 1e3, "gg_diagnostics_gbs": gbs(t_diag),
+                      "gg_diagnostics_frac": gbs(t_diag) / peak_gbs,
+                      "gg_diagnostics_noalloc_ms": t_na * 1e3, "gg_diagnostics_noalloc_gbs": gbs(t_na),
+                      "gg_diagnostics_noalloc_frac": gbs(t_na) / peak_gbs,
+                      "gg_diagnostics_noalloc_matches_gg_diagnostics": na_same,
+                      "gg_max_stable_dt_ms": t_dtmax * 1e3,
+                      "gg_max_stable_dt_note": "lambda_max(A) is reduced once by gg_set_tensor and cached on the device: "
+                                               "this call is one 64-byte read-back",
+                      "gg_step_adaptive_every_4_glups": cells * K / (float(np.median(ad)) * 1e-3) / 1e9,
+                      "gg_step_adaptive_every_4_vs_fixed": cells * K / (float(np.median(ad)) * 1e-3) / 1e9 / value}
     sim.close()
     return dict(value=value, ms=ms / K, reps_ms=reps, launches=launches, e2e=e2e,
                 clocks=clk.summary(), kernel=kernel, kernel_name=kernel_name, final=final,
@@ -404,6 +436,7 @@ def other_configs(device, wl3, only=None):
     import torch
     from paper_2006_01748_b200 import binding, workloads
     out = {}
+    peak, _ = measured_peak()
     plan = [("cfg3_f32", lambda: wl3, "f32", 40), ("cfg2_d10", lambda: workloads.make(2, d=10.0), "f64", 200),
             ("cfg4_batch64", lambda: workloads.make(4), "f64", 40), ("cfg1", lambda: workloads.make(1), "f64", 400),
             ("cfg0", lambda: workloads.make(0), "f64", 200)]
@@ -421,9 +454,20 @@ def other_configs(device, wl3, only=None):
                 ms.append(sim.last_step_ms())
             torch.cuda.synchronize(device)
             t = float(np.median(ms))
+            glups = wl.cells * K / (t * 1e-3) / 1e9
+            # algorithmic bytes per cell-step: U, V, W read and written, the three tensor fields read
+            # once per step and shared by the whole batch
+            es = 8 if dtype == "f64" else 4
+            bpc = (6.0 + 3.0 / wl.batch) * es
             out[name] = {"workload": wl.name, "dtype": dtype, "steps": K, "kernel": sim.kernel,
-                         "kernel_name": sim.kernel_name, "glups": wl.cells * K / (t * 1e-3) / 1e9,
-                         "us_per_step": t * 1e3 / K, "parity_window_max_abs_err": err,
+                         "kernel_name": sim.kernel_name, "glups": glups,
+                         "us_per_step": t * 1e3 / K,
+                         "roofline": {"bound": "hbm", "achieved": glups * bpc, "peak": peak, "unit": "GB/s",
+                                      "frac": glups * bpc / peak, "algorithmic_bytes_per_cell_step": bpc,
+                                      "traffic": None,
+                                      "note": "k-step kernels cross HBM once per k steps, so frac may exceed 1; "
+                                              "grids that stay on chip (cfg0, cfg1) are latency-bound, not HBM-bound"},
+                         "parity_window_max_abs_err": err,
                          "tolerance": 1e-10 if dtype == "f64" else 2e-4}
         log(f"config {name}: {out[name]}")
         del wl
@@ -493,8 +537,10 @@ def main():
                     help="run ONE entry of the `configs` object (cfg3_f32, cfg2_d10, cfg4_batch64, cfg1, cfg0, "
                          "ext3d_f64, ext3d_f32), print it as a JSON line and exit: the short command the ncu "
                          "captures of those kernels are taken with")
-    ap.add_argument("--extras", action="store_true",
-                    help="also time gg_diagnostics / gg_step_adaptive (adds a `reductions` object)")
+    ap.add_argument("--extras", action="store_true", help="(default since round 3; kept so that old commands still parse)")
+    ap.add_argument("--no-extras", dest="no_extras", action="store_true",
+                    help="skip the `reductions` object (gg_diagnostics, gg_diagnostics_noalloc, gg_max_stable_dt and "
+                         "gg_step_adaptive timed next to the step; costs about a second)")
     ap.add_argument("--record-traffic", default=None, metavar="RAW.csv",
                     help="update profiles/ncu_traffic.json from an `ncu --page raw --csv` dump and exit")
     args = ap.parse_args()

@@ -46,11 +46,25 @@ enum {
     GG3_KERNEL_TILED = 2     /* xy tiles marched along z, planes staged in shared memory             */
 };
 enum {
-    GG3_OPT_KERNEL = 0
+    GG3_OPT_KERNEL = 0,      /* one of GG3_KERNEL_*                                                   */
+    GG3_OPT_GRAPH = 1,       /* 1 (default): gg3_step replays cached CUDA graphs of up to              */
+                             /* GG3_OPT_GRAPH_CHUNK launches (keyed by length, ping-pong parity, kernel */
+                             /* and dt); 0: one host launch per step                                   */
+    GG3_OPT_GRAPH_CHUNK = 2  /* launches per captured graph (default 64, 1..4096)                      */
 };
 
 /* One simulation on an nx x ny x nz grid (each >= 2), spacings dx, dy, dz > 0; r, d, alpha, c: the
- * scalars of eq. (1) (c is the reaction rate the paper calls c).  HOST call. */
+ * scalars of eq. (1) (c is the reaction rate the paper calls c).  They must be finite;
+ * their signs are not policed (as in gg_create: a negative rate is the caller's business).  HOST call.
+ * The message of a failed gg3_create is per host thread (gg3_last_error(NULL)).
+ *
+ * Step size.  This interface has no gg3_max_stable_dt (and no device-side clock, diagnostics or
+ * batching: those exist for the 2-D path, gg.h).  dt is the caller's; for the linear part of the
+ * scheme the explicit bound in three dimensions is
+ *     dt <= safety * min(dx,dy,dz)^2 / max(alpha, lambda_max(A)),   safety <= 1/6
+ * (2-D: 1/4), lambda_max the largest eigenvalue of A over all cells -- a Gershgorin row sum
+ * max_p (a_pp + sum_{q != p} |a_pq|) is a safe stand-in.  The seeded recipe
+ * (paper_2006_01748_b200/workloads.py: dt_rule3) uses that row sum with safety 0.12. */
 int gg3_create(gg3_ctx** out, int nx, int ny, int nz, double dx, double dy, double dz, double r,
                double d, double alpha, double c, int dtype);
 
@@ -74,7 +88,9 @@ int gg3_set_tensor_host(gg3_ctx* ctx, const void* axx, const void* ayy, const vo
 int gg3_set_state(gg3_ctx* ctx, const void* U, const void* V, const void* W);
 int gg3_set_state_host(gg3_ctx* ctx, const void* U, const void* V, const void* W);
 
-/* n >= 0 explicit Euler steps of eq. (3) in three dimensions with step size dt > 0 (finite). */
+/* n >= 0 explicit Euler steps of eq. (3) in three dimensions with step size dt > 0 (finite).  If the
+ * call fails with GG_ERR_CUDA after its first launch the context drops its state (gg3_set_state
+ * again). */
 int gg3_step(gg3_ctx* ctx, long long n, double dt);
 
 /* Copy the current state out: DEVICE (resp. HOST, synchronising) arrays [nz][ny][nx]. */
@@ -84,8 +100,11 @@ int gg3_get_state_host(gg3_ctx* ctx, void* U, void* V, void* W);
 int gg3_set_option(gg3_ctx* ctx, int option, long long value);
 /* The kernel gg3_step runs for this context (a GG3_KERNEL_* value other than AUTO). */
 int gg3_kernel_used(const gg3_ctx* ctx);
-/* Kernel launches enqueued by gg3_step so far. */
+/* Kernel launches enqueued by gg3_step so far (graph replays count every kernel node). */
 long long gg3_launches(const gg3_ctx* ctx);
+/* CUDA graphs this context has captured so far (a loop with a fixed dt captures each chunk length
+ * and parity once; a new dt captures anew: the 3-D kernels take their coefficients by value). */
+long long gg3_graph_captures(const gg3_ctx* ctx);
 /* Device time of the last gg3_step call in milliseconds (CUDA events on the bound stream);
  * synchronises on the second event. */
 int gg3_last_step_ms(gg3_ctx* ctx, float* ms);

@@ -10,7 +10,7 @@ from . import binding as _b
 
 _vp = ctypes.c_void_p
 GG3_KERNEL_AUTO, GG3_KERNEL_GENERIC, GG3_KERNEL_TILED = range(3)
-GG3_OPT_KERNEL = 0
+GG3_OPT_KERNEL, GG3_OPT_GRAPH, GG3_OPT_GRAPH_CHUNK = range(3)
 KERNEL_NAMES = {GG3_KERNEL_GENERIC: "generic", GG3_KERNEL_TILED: "tiled"}
 
 SIGNATURES = {
@@ -27,6 +27,7 @@ SIGNATURES = {
     "gg3_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_longlong]),
     "gg3_kernel_used": (ctypes.c_int, [_vp]),
     "gg3_launches": (ctypes.c_longlong, [_vp]),
+    "gg3_graph_captures": (ctypes.c_longlong, [_vp]),
     "gg3_last_step_ms": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_float)]),
     "gg3_destroy": (ctypes.c_int, [_vp]),
     "gg3_last_error": (ctypes.c_char_p, [_vp]),
@@ -105,6 +106,10 @@ def gg3_launches(ctx) -> int:
     return int(load().gg3_launches(ctx))
 
 
+def gg3_graph_captures(ctx) -> int:
+    return int(load().gg3_graph_captures(ctx))
+
+
 def gg3_last_step_ms(ctx) -> float:
     ms = ctypes.c_float()
     _check(ctx, load().gg3_last_step_ms(ctx, ctypes.byref(ms)))
@@ -172,6 +177,10 @@ class Simulation3:
     @property
     def launches(self) -> int:
         return gg3_launches(self.ctx)
+
+    @property
+    def graph_captures(self) -> int:
+        return gg3_graph_captures(self.ctx)
 
     def last_step_ms(self) -> float:
         return gg3_last_step_ms(self.ctx)

@@ -6,13 +6,27 @@
 #include <cstdarg>
 #include <algorithm>
 #include <cstdio>
+#include <cstring>
+#include <map>
 #include <new>
 #include <string>
+#include <tuple>
 
 #include "../../include/gg.h"
 #include "../../include/gg3.h"
 #include "gg3_kernels.cuh"
 #include "gg3_tiled.cuh"
+
+// A captured run of gg3_step launches.  The 3-D kernels take their folded coefficients BY VALUE
+// (Args3::k), so unlike the 2-D graphs these are keyed by dt as well (its bit pattern).
+struct Graph3Key {
+    long long len;
+    int parity, kernel;
+    unsigned long long dt_bits;
+    bool operator<(const Graph3Key& o) const {
+        return std::tie(len, parity, kernel, dt_bits) < std::tie(o.len, o.parity, o.kernel, o.dt_bits);
+    }
+};
 
 struct gg3_ctx {
     int nx = 0, ny = 0, nz = 0, dtype = GG_F64;
@@ -25,6 +39,11 @@ struct gg3_ctx {
     int cur = 0;
     bool bound = false, have_tensor = false, have_state = false, timed = false;
     int opt_kernel = GG3_KERNEL_AUTO;
+    int opt_graph = 1;           // GG3_OPT_GRAPH
+    long long opt_chunk = 64;    // GG3_OPT_GRAPH_CHUNK
+    std::map<Graph3Key, cudaGraphExec_t> graphs;
+    long long graph_captures = 0;
+    int num_sms = 148;           // of the device current at gg3_bind (sizes the grids)
     long long launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     mutable std::string err;
@@ -34,7 +53,7 @@ struct gg3_ctx {
 
 namespace {
 
-std::string g3_create_error;
+thread_local std::string g3_create_error;   // per thread, like gg_api.cu's: concurrent failing gg3_create calls do not race
 
 int fail3(const gg3_ctx* c, int code, const char* fmt, ...) {
     char buf[512];
@@ -84,7 +103,7 @@ int launch_step(gg3_ctx* c, int kernel, int src, double dt) {
     if (kernel == GG3_KERNEL_TILED) {
         const dim3 block(gg3::kTileX, gg3::kTileY);
         const dim3 grid((c->nx + gg3::kTileX - 1) / gg3::kTileX, (c->ny + gg3::kTileY - 1) / gg3::kTileY,
-                        gg3::tiled_zchunks(c->nx, c->ny, c->nz));
+                        gg3::tiled_zchunks(c->nx, c->ny, c->nz, c->num_sms));
         gg3::gg3_step_tiled<T><<<grid, block, gg3::tiled_smem_bytes<T>(), c->stream>>>(a);
     } else {
         const dim3 block(32, 4, 2);
@@ -93,6 +112,48 @@ int launch_step(gg3_ctx* c, int kernel, int src, double dt) {
     }
     GG3_CUDA(c, cudaGetLastError());
     return GG_OK;
+}
+
+void drop_graphs3(gg3_ctx* c) {
+    for (auto& kv : c->graphs) cudaGraphExecDestroy(kv.second);
+    c->graphs.clear();
+}
+
+// `len` plain launches from copy `src` on c->stream (ping-pong); the caller flips c->cur.
+int enqueue_steps3(gg3_ctx* c, int kernel, int src, long long len, double dt) {
+    for (long long s = 0; s < len; ++s, src ^= 1) {
+        const int rc = c->dtype == GG_F64 ? launch_step<double>(c, kernel, src, dt) : launch_step<float>(c, kernel, src, dt);
+        if (rc) return rc;
+    }
+    return GG_OK;
+}
+
+// Capture `len` steps starting at copy `src` into an executable graph (on a private capture stream;
+// thread-local capture mode, so other threads' CUDA calls are not disturbed).
+int capture_graph3(gg3_ctx* c, int kernel, int src, long long len, double dt, cudaGraphExec_t* out) {
+    cudaStream_t cap = nullptr;
+    GG3_CUDA(c, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = c->stream;
+    c->stream = cap;
+    cudaGraph_t graph = nullptr;
+    int rc = GG_OK;
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) {
+        rc = fail3(c, GG_ERR_CUDA, "cudaStreamBeginCapture: %s", cudaGetErrorString(e));
+    } else {
+        rc = enqueue_steps3(c, kernel, src, len, dt);
+        e = cudaStreamEndCapture(cap, &graph);
+        if (rc == GG_OK && e != cudaSuccess) rc = fail3(c, GG_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    }
+    c->stream = user;
+    if (rc == GG_OK) {
+        e = cudaGraphInstantiate(out, graph, 0);
+        if (e != cudaSuccess) rc = fail3(c, GG_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+        else ++c->graph_captures;
+    }
+    if (graph) cudaGraphDestroy(graph);
+    cudaStreamDestroy(cap);
+    return rc;
 }
 
 template <typename F>
@@ -138,6 +199,9 @@ int gg3_bind(gg3_ctx* ctx, void* ws, size_t bytes, void* stream) {
     if (!ws || ((size_t)ws & 255)) return fail3(ctx, GG_ERR_ARG, "gg3_bind: workspace must be non-NULL and 256-byte aligned");
     if (bytes < gg3_workspace_bytes(ctx)) return fail3(ctx, GG_ERR_ARG, "gg3_bind: workspace too small");
     if (ctx->bound) return fail3(ctx, GG_ERR_STATE, "gg3_bind: already bound");
+    int dev = 0;
+    GG3_CUDA(ctx, cudaGetDevice(&dev));
+    GG3_CUDA(ctx, cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev));
     ctx->ws = (char*)ws; ctx->ws_bytes = bytes; ctx->stream = (cudaStream_t)stream;
     size_t off = 0;
     for (int p = 0; p < 2; ++p)
@@ -161,7 +225,7 @@ static int set_tensor3(gg3_ctx* ctx, const void* const src[6], bool host) {
     // the entries as given are staged in the ping-pong copy that holds no live time level, three at
     // a time (the stored form of an entry needs its neighbour along one axis)
     void* scratch[3] = {ctx->state[ctx->cur ^ 1][0], ctx->state[ctx->cur ^ 1][1], ctx->state[ctx->cur ^ 1][2]};
-    const int blocks = (int)std::min<size_t>((ctx->cells() + 255) / 256, (size_t)148 * 8);
+    const int blocks = (int)std::min<size_t>((ctx->cells() + 255) / 256, (size_t)ctx->num_sms * 8);
     const double sc[6] = {0.5 / (ctx->dx * ctx->dx), 0.5 / (ctx->dy * ctx->dy), 0.5 / (ctx->dz * ctx->dz),
                           0.25 / (ctx->dx * ctx->dy), 0.25 / (ctx->dx * ctx->dz), 0.25 / (ctx->dy * ctx->dz)};
     for (int f = 0; f < 6; ++f) {
@@ -223,20 +287,55 @@ int gg3_step(gg3_ctx* ctx, long long n, double dt) {
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail3(ctx, GG_ERR_ARG, "gg3_step: dt must be finite and > 0");
     if (n == 0) return GG_OK;
     const int kernel = resolve3(ctx);
-    GG3_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-    for (long long s = 0; s < n; ++s) {
-        const int rc = ctx->dtype == GG_F64 ? launch_step<double>(ctx, kernel, ctx->cur, dt) : launch_step<float>(ctx, kernel, ctx->cur, dt);
-        if (rc) { ctx->have_state = false; return rc; }
-        ctx->cur ^= 1;
-        ctx->launches += 1;
-    }
-    GG3_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
-    ctx->timed = true;
-    return GG_OK;
+    return guarded3(ctx, "gg3_step", [&]() -> int {
+        GG3_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+        long long left = n;
+        unsigned long long dt_bits = 0;
+        std::memcpy(&dt_bits, &dt, sizeof dt_bits);
+        while (left > 0) {
+            // the step loop is replayed from cached graphs of up to opt_chunk launches (one host call
+            // per chunk instead of one per step: small grids are launch-bound otherwise)
+            const long long len = ctx->opt_graph && n >= 2 ? (left < ctx->opt_chunk ? left : ctx->opt_chunk) : left;
+            int rc = GG_OK;
+            if (ctx->opt_graph && n >= 2) {
+                const Graph3Key key{len, ctx->cur, kernel, dt_bits};
+                auto it = ctx->graphs.find(key);
+                if (it == ctx->graphs.end()) {
+                    if (ctx->graphs.size() >= 16) drop_graphs3(ctx);
+                    cudaGraphExec_t ex = nullptr;
+                    rc = capture_graph3(ctx, kernel, ctx->cur, len, dt, &ex);
+                    if (rc == GG_OK) it = ctx->graphs.emplace(key, ex).first;
+                }
+                if (rc == GG_OK) {
+                    const cudaError_t e = cudaGraphLaunch(it->second, ctx->stream);
+                    if (e != cudaSuccess) rc = fail3(ctx, GG_ERR_CUDA, "cudaGraphLaunch: %s", cudaGetErrorString(e));
+                }
+            } else {
+                rc = enqueue_steps3(ctx, kernel, ctx->cur, len, dt);
+            }
+            if (rc) { ctx->have_state = false; return rc; }   // some launches may be enqueued: no consistent time level
+            ctx->cur ^= (int)(len & 1);
+            ctx->launches += len;
+            left -= len;
+        }
+        GG3_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+        ctx->timed = true;
+        return GG_OK;
+    });
 }
 
 int gg3_set_option(gg3_ctx* ctx, int option, long long value) {
     if (!ctx) return GG_ERR_ARG;
+    if (option == GG3_OPT_GRAPH) {
+        if (value != 0 && value != 1) return fail3(ctx, GG_ERR_ARG, "GG3_OPT_GRAPH: 0 or 1");
+        ctx->opt_graph = (int)value;
+        return GG_OK;
+    }
+    if (option == GG3_OPT_GRAPH_CHUNK) {
+        if (value < 1 || value > 4096) return fail3(ctx, GG_ERR_ARG, "GG3_OPT_GRAPH_CHUNK: 1..4096");
+        ctx->opt_chunk = value;
+        return GG_OK;
+    }
     if (option != GG3_OPT_KERNEL) return fail3(ctx, GG_ERR_UNSUPPORTED, "gg3_set_option: unknown option %d", option);
     if (value != GG3_KERNEL_AUTO && value != GG3_KERNEL_GENERIC && value != GG3_KERNEL_TILED)
         return fail3(ctx, GG_ERR_UNSUPPORTED, "gg3_set_option: kernel %lld not available", value);
@@ -247,6 +346,7 @@ int gg3_set_option(gg3_ctx* ctx, int option, long long value) {
 }
 int gg3_kernel_used(const gg3_ctx* ctx) { return ctx ? resolve3(ctx) : -1; }
 long long gg3_launches(const gg3_ctx* ctx) { return ctx ? ctx->launches : 0; }
+long long gg3_graph_captures(const gg3_ctx* ctx) { return ctx ? ctx->graph_captures : 0; }
 int gg3_last_step_ms(gg3_ctx* ctx, float* ms) {
     if (!ctx || !ms) return GG_ERR_ARG;
     if (!ctx->timed) return fail3(ctx, GG_ERR_STATE, "gg3_last_step_ms: no gg3_step call yet");
@@ -257,6 +357,7 @@ int gg3_last_step_ms(gg3_ctx* ctx, float* ms) {
 int gg3_destroy(gg3_ctx* ctx) {
     if (!ctx) return GG_OK;
     if (ctx->bound) cudaStreamSynchronize(ctx->stream);
+    drop_graphs3(ctx);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;

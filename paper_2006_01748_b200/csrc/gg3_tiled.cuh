@@ -36,9 +36,9 @@ static_assert(kHalo <= kTileX * kTileY, "one halo cell per thread at most");
 __host__ __device__ inline bool tiled_shape_ok(int nx, int ny, int nz) { return nx >= 2 && ny >= 2 && nz >= 2; }
 // chunks along z: enough CTAs to fill the GPU several times over, but at least 8 planes per chunk
 // (every chunk re-reads two planes of W and one of everything else)
-__host__ __device__ inline int tiled_zchunks(int nx, int ny, int nz) {
+__host__ __device__ inline int tiled_zchunks(int nx, int ny, int nz, int num_sms) {
     const long long tiles = (long long)((nx + kTileX - 1) / kTileX) * ((ny + kTileY - 1) / kTileY);
-    long long want = (148LL * 16 + tiles - 1) / tiles;
+    long long want = ((long long)num_sms * 16 + tiles - 1) / tiles;
     const long long most = nz / 8 > 0 ? nz / 8 : 1;
     if (want > most) want = most;
     if (want < 1) want = 1;

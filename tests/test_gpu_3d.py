@@ -62,6 +62,36 @@ def test_config_recipe_long_run_and_kernels_bit_identical():
     assert ref[2].max() > 0.05 and ref[0].min() < 0.5
 
 
+def test_graph_replay_is_bit_identical_to_plain_launches_and_caches_by_dt():
+    """gg3_step replays cached CUDA graphs (GG3_OPT_GRAPH, default on).  Odd and even chunk
+    lengths, a ragged last chunk, split calls: the end state equals the plain-launch loop bit for
+    bit; a loop with one dt captures each (length, parity) once, a second dt captures anew (the 3-D
+    kernels take their coefficients by value)."""
+    wl = workloads.make3d(70, 21, 24, steps=37, random_state=True)
+    with binding3.from_workload(wl) as sim:
+        sim.set_option(binding3.GG3_OPT_GRAPH, 0)
+        sim.step(wl.steps, wl.dt)
+        sim.step(5, 0.5 * wl.dt)
+        plain = sim.get_state_numpy()
+        assert sim.graph_captures == 0 and sim.launches == 42
+    with binding3.from_workload(wl) as sim:
+        sim.set_option(binding3.GG3_OPT_GRAPH_CHUNK, 7)       # 37 = 5 x 7 + 2: parities alternate
+        sim.step(wl.steps, wl.dt)
+        caps = sim.graph_captures
+        assert caps == 3                                      # (7, parity 0), (7, parity 1), (2, parity 1)
+        sim.step(5, 0.5 * wl.dt)                              # new dt: one more capture
+        assert sim.graph_captures == caps + 1 and sim.launches == 42
+        graph = sim.get_state_numpy()
+        sim.step(5, 0.5 * wl.dt)                              # same key, other parity
+        sim.step(5, 0.5 * wl.dt)                              # cached
+        assert sim.graph_captures == caps + 2
+    for x, y in zip(plain, graph):
+        assert np.array_equal(x, y)
+    assert_close(graph, oracle.step3d(*oracle_run(wl, wl.steps), wl.tensor, r=wl.r, d=wl.d, alpha=wl.alpha,
+                                      c_r=wl.c_r, n=5, dt=0.5 * wl.dt, dx=wl.dx, dy=wl.dy, dz=wl.dz),
+                 "f64", "graph replay, two step sizes")
+
+
 def test_anisotropic_mesh():
     wl = workloads.make3d(40, 24, 20, spacing=(1 / 64, 1 / 48, 1 / 80), random_state=True)
     for kernel in ("generic", "tiled"):

@@ -82,3 +82,36 @@ def test_onchip_kernels_many_calls_bit_identical():
         for x, y in zip(*outs):
             assert np.array_equal(x, y), f"on-chip kernel differs from stream: {nx}x{ny}x{b} {dtype}"
     assert ncase >= 8
+
+
+def test_cluster_kernel_stress_thin_slabs_long_calls_many_clusters():
+    """The cluster kernel's halo protocol (remote st.async rows completed on the receiver's
+    mbarrier, two state copies reused every second step on the argument that a neighbour is at most
+    one step ahead) where it is most exposed: ONE row per CTA and grids with fewer rows than the
+    cluster has CTAs (some CTAs own nothing), both cluster sizes, batches of 40 and 75 simulations
+    (more clusters than the GPU holds at once, so waves of clusters start and finish at different
+    times), and thousands of steps inside a single launch.  Bit for bit against the single-step
+    kernel: a hand-off that is lost, early or late changes bits."""
+    cases = [  # nx, ny, batch, dtype, cluster CTAs (0 = the library's choice), steps per call
+        (32, 16, 1, "f64", 16, (3000, 1)),     # R = 1 with every CTA busy
+        (64, 5, 40, "f64", 8, (1501, 2)),      # ny < CL: three CTAs of every cluster own no row
+        (16, 2, 75, "f32", 16, (2000,)),       # two rows in a 16-CTA cluster, 75 clusters
+        (128, 9, 40, "f32", 8, (999, 64)),     # R = 2, the last CTAs ragged / empty
+        (96, 33, 9, "f64", 0, (1200, 7)),
+    ]
+    for nx, ny, b, dtype, ctas, calls in cases:
+        wl = workloads.random_problem(7000 + nx + ny, nx, ny, batch=b)
+        outs = []
+        for kern in ("resident", "stream"):
+            with B.from_workload(wl, dtype=dtype) as sim:
+                sim.set_option(B.GG_OPT_KERNEL, KERNELS[kern])
+                if kern == "resident" and ctas:
+                    sim.set_option(B.GG_OPT_CLUSTER_CTAS, ctas)
+                for n in calls:
+                    sim.step(n, wl.dt)
+                    if kern == "resident":
+                        assert "gg_step_cluster" in sim.kernel_name, sim.kernel_name
+                outs.append(sim.get_state_numpy())
+        for x, y in zip(*outs):
+            assert np.isfinite(x).all()
+            assert np.array_equal(x, y), f"cluster kernel differs from stream: {nx}x{ny}x{b} {dtype} CL={ctas}"
