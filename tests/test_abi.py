@@ -147,6 +147,25 @@ def test_options_validate():
         binding.gg_destroy(ctx)
 
 
+def test_noalloc_entry_point_validates_before_touching_the_device():
+    """gg_diagnostics_noalloc checks its arguments before any CUDA call, so the refusals can be
+    seen without a GPU: a batch beyond the built-in scratch, NULL arrays, bad sizes."""
+    nb = binding.GG_NOALLOC_MAX_BATCH
+    fake = 4096                                         # never dereferenced: validation fails first
+    with pytest.raises(binding.GGError) as e:
+        binding.gg_diagnostics_noalloc(fake, fake, fake, nb + 1, 8, 8, binding.GG_F64, 0.1, fake, 0)
+    assert e.value.code == binding.GG_ERR_ARG and "GG_NOALLOC_MAX_BATCH" in str(e.value)
+    for args in ((0, fake, fake, 1, 8, 8, binding.GG_F64, 0.1, fake), (fake, fake, fake, 1, 8, 8, binding.GG_F64, 0.1, 0),
+                 (fake, fake, fake, 0, 8, 8, binding.GG_F64, 0.1, fake), (fake, fake, fake, 1, 8, 0, binding.GG_F64, 0.1, fake),
+                 (fake, fake, fake, 1, 8, 8, binding.GG_F64, -1.0, fake), (fake + 4, fake, fake, 1, 8, 8, binding.GG_F64, 0.1, fake)):
+        with pytest.raises(binding.GGError) as e:
+            binding.gg_diagnostics_noalloc(*args, 0)
+        assert e.value.code == binding.GG_ERR_ARG and binding.gg_noalloc_last_error()
+    with pytest.raises(binding.GGError) as e:
+        binding.gg_diagnostics_noalloc(fake, fake, fake, 1, 8, 8, 9, 0.1, fake, 0)
+    assert e.value.code == binding.GG_ERR_UNSUPPORTED
+
+
 def test_no_cpu_fallback_without_device():
     import torch
     if torch.cuda.is_available():
